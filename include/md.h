@@ -1,0 +1,135 @@
+/* md.h -- C ABI of the B200-native many-body force library (arXiv 1610.03343 hot path).
+ *
+ * Write-conflict-free force evaluation for many-body potentials:
+ *   1. periodic cell-list neighbour build
+ *   2. per-pair kernel: bond order zeta_ij, b_ij and the partial derivative
+ *      P_ij = dU_i/dr_ij of every listed pair        (Eq. 14, Alg. 3 at 295-322)
+ *   3. one-thread-per-atom gather, no atomics:
+ *        F_i = sum_j (P_ij - P_ji)                   (Eq. 28)
+ *        W_i = -1/2 sum_j r_ij (x) (P_ij - P_ji)     (Eq. 29)
+ *        J_i = sum_j r_ij (P_ji . v_i)               (Eq. 30)
+ *   4. velocity-Verlet NVE
+ *
+ * Conventions
+ *   - Units: Angstrom, fs, amu, eV; velocities in A/fs; forces in eV/A.
+ *   - r_ij = r_j - r_i, minimum image in an orthorhombic fully periodic box
+ *     (PAPER.md:272).  Coordinates must lie in [0, box[a]); md_velocity_verlet_step keeps them there.
+ *   - Unless marked HOST, every pointer is a DEVICE pointer owned by the caller.  Vectors are
+ *     structure-of-arrays: f[3][n], virial[9][n] (row-major ab, a from r, b from F: W_ab = -1/2 sum r^a F^b),
+ *     heat[3][n].  Nothing in caller arrays is permuted.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and
+ *     return without synchronising unless stated.
+ *   - Return value: MD_OK or a negative md_status.  Argument errors are detected synchronously and
+ *     have no side effects.  Conditions found on the device (a neighbour row longer than
+ *     max_neighbors, a missing reverse entry, too many in-range neighbours) latch a status word in
+ *     the handle; md_neighbors_status() synchronises the stream and returns it.
+ *   - There is no CPU fallback: every entry point needs a CUDA device.
+ */
+#ifndef MD_H_
+#define MD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MD_OK = 0,
+    MD_ERR_ARG = -1,
+    MD_ERR_ALLOC = -2,
+    MD_ERR_BOX_TOO_SMALL = -3,       /* fewer than 3 cells of edge >= r_list on some axis */
+    MD_ERR_NEIGHBOR_OVERFLOW = -4,   /* a row needs more than max_neighbors entries */
+    MD_ERR_CUDA = -5,
+    MD_ERR_NO_LIST = -6,             /* force call before a list was built or imported */
+    MD_ERR_LIST_ASYMMETRIC = -7      /* j in row i but i not in row j (imported list) */
+} md_status;
+
+enum { MD_FP64 = 0, MD_FP32 = 1 };          /* arithmetic of the force kernels (reading A10) */
+enum { MD_TERSOFF = 0, MD_SW = 1 };
+enum { MD_MAX_NEIGHBORS = 64 };
+
+/* Tersoff parameters, single element (Eqs. 1-6); HOST struct, copied by the call.
+ * f_R = A exp(-lambda r), f_A = B exp(-mu r), f_C: 1 below R, cosine taper to 0 at S. */
+typedef struct { double A, B, lambda, mu, beta, n, c, d, h, R, S; } md_tersoff_params;
+
+/* Stillinger-Weber parameters (Ref. [18]); cutoff r_c = a*sigma; cos0 = -1/3 for Si. */
+typedef struct { double epsilon, sigma, a, lambda, gamma, A, B, p, q, cos0; } md_sw_params;
+
+/* Opaque handle: library-owned device scratch (cell arrays, NN, NL, reverse index, per-pair records). */
+typedef struct md_neighbors md_neighbors;
+
+/* Create / destroy the handle for up to n_atoms atoms and rows of up to max_neighbors
+ * (1..MD_MAX_NEIGHBORS) entries.  Allocates device memory (synchronous). */
+int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors);
+int md_neighbors_destroy(md_neighbors* nl);
+
+/* Synchronises `stream`, returns the latched device status (MD_OK if none) and clears it.
+ * max_count_seen (HOST, may be NULL) receives the longest row of the last build. */
+int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream);
+
+/* Copy the current list out / in (DEVICE int32 buffers): NN[n]; NL[max_neighbors][n] neighbour-major,
+ * NL[m*n + i] = index of the m-th neighbour of atom i, rows sorted by index.
+ * Import also rebuilds the reverse index; it lets a test drive the force kernels with an
+ * externally built list. */
+int md_neighbors_export(md_neighbors* nl, int32_t* NN, int32_t* NL, void* stream);
+int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const int32_t* NL, void* stream);
+
+/* Step 1.  Verlet list by the cell-list method: all j != i with minimum-image
+ * d2 = fma(dz,dz,fma(dy,dy,dx*dx)) < r_list*r_list (strict; reading A7).
+ * box: HOST double[3].  Needs floor(box[a]/r_list) >= 3 on every axis. */
+int md_build_neighbors(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                       const double box[3], double r_list, void* stream);
+
+/* Steps 2+3 for the Tersoff potential.  vx,vy,vz are read only when heat != NULL.
+ * Outputs (any may be NULL): pe[n] = U_i, f[3][n], virial[9][n], heat[3][n].
+ * precision: MD_FP64 or MD_FP32 (float arithmetic on r_ij formed in double; outputs stay double). */
+int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                     const double* vx, const double* vy, const double* vz, const double box[3],
+                     const md_tersoff_params* p, int precision,
+                     double* pe, double* f, double* virial, double* heat, void* stream);
+
+/* Same for Stillinger-Weber; three-body energy is attributed to the central atom (reading A6). */
+int md_sw_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                const double* vx, const double* vy, const double* vz, const double box[3],
+                const md_sw_params* p, int precision,
+                double* pe, double* f, double* virial, double* heat, void* stream);
+
+/* Step 4.  One half of a velocity-Verlet step, in place.
+ *   phase 0: v += (dt/2)(kappa/m) f ; x += dt v ; wrap into [0, box)
+ *   phase 1: v += (dt/2)(kappa/m) f
+ * kappa = 9.648533215665e-3 (A/fs^2)/(eV/A/amu). */
+int md_velocity_verlet_step(int phase, int64_t n, double* x, double* y, double* z,
+                            double* vx, double* vy, double* vz, const double* f,
+                            double mass_amu, double dt_fs, const double box[3], void* stream);
+
+/* Convenience: nsteps NVE steps composed of the four calls above, list rebuilt after the drift of
+ * every step s with s % rebuild_every == 0.  `params` is a HOST md_tersoff_params* or md_sw_params*
+ * according to `potential`.  f[3][n] must hold the forces of the incoming state if f_valid != 0,
+ * otherwise they are computed first (with a list built at the incoming positions).
+ * pe[n] (may be NULL) receives U_i of the final state. */
+int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+               double* x, double* y, double* z, double* vx, double* vy, double* vz,
+               double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
+               int nsteps, int rebuild_every, double r_list, void* stream);
+
+/* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
+ * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
+ * synchronises.  Device buffers are owned by the handle. */
+int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+                    double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                    double* f, double* pe, const double box[3], double mass_amu, double dt_fs,
+                    int nsteps, int rebuild_every, double r_list, void* stream);
+
+/* Diagnostic: runs an independent-chain DFMA kernel for `iters` fused multiply-adds per thread on a
+ * full grid and returns the achieved FP64 rate in *tflops (HOST); used as the measured ALU peak of
+ * the roofline.  Synchronous. */
+int md_probe_fp64_peak(int iters, double* tflops, void* stream);
+
+/* Library version string (HOST, static storage). */
+const char* md_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_H_ */

@@ -1,0 +1,217 @@
+// api.cu -- the C ABI declared in include/md.h: argument checks, handle life cycle, and the host-side
+// composition of the kernels.  No arithmetic of the method lives here.
+#include <new>
+
+#include "common.cuh"
+
+namespace {
+
+bool valid_box(const double box[3]) { return box && box[0] > 0 && box[1] > 0 && box[2] > 0; }
+
+void free_all(md_neighbors* nl) {
+    cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
+    cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted);
+    cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e);
+}
+
+int force_dispatch(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+                   const double* x, const double* y, const double* z, const double* vx, const double* vy,
+                   const double* vz, const double box[3], double* pe, double* f, double* virial,
+                   double* heat, cudaStream_t s) {
+    if (potential == MD_TERSOFF)
+        return md_launch_tersoff(nl, n, x, y, z, vx, vy, vz, box, (const md_tersoff_params*)params, precision,
+                                 pe, f, virial, heat, s);
+    return md_launch_sw(nl, n, x, y, z, vx, vy, vz, box, (const md_sw_params*)params, precision, pe, f,
+                        virial, heat, s);
+}
+
+int check_force_args(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                     const double* vx, const double* vy, const double* vz, const double box[3],
+                     const void* p, int precision, const double* heat) {
+    if (!nl || n < 0 || !valid_box(box) || !p) return MD_ERR_ARG;
+    if (precision != MD_FP64 && precision != MD_FP32) return MD_ERR_ARG;
+    if (n > 0 && (!x || !y || !z)) return MD_ERR_ARG;
+    if (heat && n > 0 && (!vx || !vy || !vz)) return MD_ERR_ARG;
+    if (nl->n != n) return MD_ERR_NO_LIST;
+    return MD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* md_version(void) { return "paper_1610_03343_b200 0.1 (sm_100a)"; }
+
+int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) {
+    if (!out || n_atoms < 0 || max_neighbors < 1 || max_neighbors > MD_MAX_NEIGHBORS) return MD_ERR_ARG;
+    if (n_atoms * (int64_t)max_neighbors > (int64_t)2000000000) return MD_ERR_ARG;   // int32 pair indices
+    md_neighbors* nl = new (std::nothrow) md_neighbors();
+    if (!nl) return MD_ERR_ALLOC;
+    *nl = md_neighbors{};
+    nl->n_cap = n_atoms; nl->K = max_neighbors;
+    const size_t n = (size_t)(n_atoms > 0 ? n_atoms : 1), K = (size_t)max_neighbors;
+    bool ok = true;
+    ok = ok && cudaMalloc(&nl->NN, n * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->NL, n * K * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->REV, n * K) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->Q, n * K * sizeof(PairRec64)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->MASK, n * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->cell_of, n * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->rank_in_cell, n * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->d_status, 2 * sizeof(int)) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); free_all(nl); delete nl; return MD_ERR_ALLOC; }
+    cudaMemset(nl->d_status, 0, 2 * sizeof(int));
+    *out = nl;
+    return MD_OK;
+}
+
+int md_neighbors_destroy(md_neighbors* nl) {
+    if (!nl) return MD_ERR_ARG;
+    cudaDeviceSynchronize();
+    free_all(nl);
+    delete nl;
+    return MD_OK;
+}
+
+int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream) {
+    if (!nl) return MD_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    int h[2] = {0, 0};
+    MD_CUDA_TRY(cudaMemcpyAsync(h, nl->d_status, sizeof(h), cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaStreamSynchronize(s));
+    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status, 0, sizeof(int), s));
+    if (max_count_seen) *max_count_seen = h[1];
+    if (h[0] & (MD_DEV_ROW_OVERFLOW | MD_DEV_INRANGE_OVERFLOW)) return MD_ERR_NEIGHBOR_OVERFLOW;
+    if (h[0] & MD_DEV_NO_REVERSE) return MD_ERR_LIST_ASYMMETRIC;
+    return MD_OK;
+}
+
+int md_neighbors_export(md_neighbors* nl, int32_t* NN, int32_t* NL, void* stream) {
+    if (!nl || !NN || !NL) return MD_ERR_ARG;
+    if (nl->n == 0) return MD_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    MD_CUDA_TRY(cudaMemcpyAsync(NN, nl->NN, sizeof(int32_t) * nl->n, cudaMemcpyDeviceToDevice, s));
+    MD_CUDA_TRY(cudaMemcpyAsync(NL, nl->NL, sizeof(int32_t) * nl->n * nl->K, cudaMemcpyDeviceToDevice, s));
+    return MD_OK;
+}
+
+int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const int32_t* NL, void* stream) {
+    if (!nl || n < 0 || n > nl->n_cap || (n > 0 && (!NN || !NL))) return MD_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    nl->n = n;
+    if (n == 0) return MD_OK;
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->NN, NN, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, s));
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->NL, NL, sizeof(int32_t) * n * nl->K, cudaMemcpyDeviceToDevice, s));
+    return md_launch_reverse(nl, s);
+}
+
+int md_build_neighbors(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                       const double box[3], double r_list, void* stream) {
+    if (!nl || n < 0 || n > nl->n_cap || !valid_box(box) || !(r_list > 0)) return MD_ERR_ARG;
+    if (n > 0 && (!x || !y || !z)) return MD_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, sizeof(int), s));
+    return md_launch_build(nl, n, x, y, z, box, r_list, s);
+}
+
+int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                     const double* vx, const double* vy, const double* vz, const double box[3],
+                     const md_tersoff_params* p, int precision,
+                     double* pe, double* f, double* virial, double* heat, void* stream) {
+    int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
+    if (rc != MD_OK) return rc;
+    if (!(p->S > p->R) || !(p->R > 0) || !(p->n > 0) || !(p->d != 0)) return MD_ERR_ARG;
+    return md_launch_tersoff(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat,
+                             (cudaStream_t)stream);
+}
+
+int md_sw_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                const double* vx, const double* vy, const double* vz, const double box[3],
+                const md_sw_params* p, int precision,
+                double* pe, double* f, double* virial, double* heat, void* stream) {
+    int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
+    if (rc != MD_OK) return rc;
+    if (!(p->sigma > 0) || !(p->a > 0)) return MD_ERR_ARG;
+    return md_launch_sw(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat,
+                        (cudaStream_t)stream);
+}
+
+int md_velocity_verlet_step(int phase, int64_t n, double* x, double* y, double* z,
+                            double* vx, double* vy, double* vz, const double* f,
+                            double mass_amu, double dt_fs, const double box[3], void* stream) {
+    if ((phase != 0 && phase != 1) || n < 0 || !(mass_amu > 0)) return MD_ERR_ARG;
+    if (n > 0 && (!vx || !vy || !vz || !f)) return MD_ERR_ARG;
+    if (phase == 0 && (!valid_box(box) || (n > 0 && (!x || !y || !z)))) return MD_ERR_ARG;
+    return md_launch_vv(phase, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, (cudaStream_t)stream);
+}
+
+int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+               double* x, double* y, double* z, double* vx, double* vy, double* vz,
+               double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
+               int nsteps, int rebuild_every, double r_list, void* stream) {
+    if (!nl || !params || n < 0 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1)
+        return MD_ERR_ARG;
+    if (potential != MD_TERSOFF && potential != MD_SW) return MD_ERR_ARG;
+    if (precision != MD_FP64 && precision != MD_FP32) return MD_ERR_ARG;
+    if (!(mass_amu > 0) || !(r_list > 0)) return MD_ERR_ARG;
+    if (n > 0 && (!x || !y || !z || !vx || !vy || !vz || !f)) return MD_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc;
+    if (!f_valid) {
+        if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 pe, f, nullptr, nullptr, s)) != MD_OK) return rc;
+    }
+    for (int step = 0; step < nsteps; ++step) {
+        if ((rc = md_launch_vv(0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if (step % rebuild_every == 0)
+            if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if (nl->n != n) return MD_ERR_NO_LIST;
+        const bool last = step == nsteps - 1;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 last ? pe : nullptr, f, nullptr, nullptr, s)) != MD_OK) return rc;
+        if ((rc = md_launch_vv(1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+    }
+    return MD_OK;
+}
+
+int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+                    double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                    double* f, double* pe, const double box[3], double mass_amu, double dt_fs,
+                    int nsteps, int rebuild_every, double r_list, void* stream) {
+    if (!nl || n < 0 || n > nl->n_cap) return MD_ERR_ARG;
+    if (n > 0 && (!x || !y || !z || !vx || !vy || !vz)) return MD_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (nl->e2e_cap < n || !nl->e2e) {
+        MD_CUDA_TRY(cudaStreamSynchronize(s));
+        if (nl->e2e) cudaFree(nl->e2e);
+        nl->e2e = nullptr; nl->e2e_cap = 0;
+        if (cudaMalloc(&nl->e2e, sizeof(double) * 10 * (size_t)(n > 0 ? n : 1)) != cudaSuccess) {
+            cudaGetLastError();
+            return MD_ERR_ALLOC;
+        }
+        nl->e2e_cap = n;
+    }
+    double* d = nl->e2e;
+    double* host_in[6] = {x, y, z, vx, vy, vz};
+    const size_t bytes = sizeof(double) * (size_t)n;
+    for (int a = 0; a < 6; ++a)
+        MD_CUDA_TRY(cudaMemcpyAsync(d + a * n, host_in[a], bytes, cudaMemcpyHostToDevice, s));
+    int rc = md_nve_run(nl, potential, params, precision, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n,
+                        d + 6 * n, 0, d + 9 * n, box, mass_amu, dt_fs, nsteps, rebuild_every, r_list, stream);
+    if (rc != MD_OK) return rc;
+    for (int a = 0; a < 6; ++a)
+        MD_CUDA_TRY(cudaMemcpyAsync(host_in[a], d + a * n, bytes, cudaMemcpyDeviceToHost, s));
+    if (f) MD_CUDA_TRY(cudaMemcpyAsync(f, d + 6 * n, 3 * bytes, cudaMemcpyDeviceToHost, s));
+    if (pe) MD_CUDA_TRY(cudaMemcpyAsync(pe, d + 9 * n, bytes, cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaStreamSynchronize(s));
+    return MD_OK;
+}
+
+int md_probe_fp64_peak(int iters, double* tflops, void* stream) {
+    if (iters < 1 || !tflops) return MD_ERR_ARG;
+    return md_launch_probe_fp64(iters, tflops, (cudaStream_t)stream);
+}
+
+}  // extern "C"

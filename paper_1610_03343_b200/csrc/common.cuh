@@ -1,0 +1,76 @@
+// common.cuh -- handle layout and small device helpers shared by the CUDA translation units.
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "md.h"
+
+#define MD_CUDA_TRY(expr)                         \
+    do {                                          \
+        cudaError_t e__ = (expr);                 \
+        if (e__ != cudaSuccess) return MD_ERR_CUDA; \
+    } while (0)
+
+// device-latched status bits (md_neighbors::d_status[0])
+enum : int {
+    MD_DEV_ROW_OVERFLOW = 1,     // neighbour row longer than max_neighbors
+    MD_DEV_NO_REVERSE = 2,       // i not found in row j
+    MD_DEV_INRANGE_OVERFLOW = 4  // more in-range neighbours than the pair kernel's cap
+};
+
+// 32-byte per-pair record {Px, Py, Pz, pad} = one DRAM sector (FP64 mode);
+// FP32 mode stores float4 in the first 16 bytes of a 16-byte-strided array.
+struct __align__(32) PairRec64 { double x, y, z, w; };
+
+struct md_neighbors {
+    int64_t n_cap;          // capacity in atoms
+    int64_t n;              // atoms of the current list (0 = none)
+    int K;                  // max_neighbors
+    // list
+    int32_t* NN;            // [n]
+    int32_t* NL;            // [K][n] neighbour-major
+    uint8_t* REV;           // [K][n] position of i in row NL[m][i]
+    // per-pair records, pushed layout: Q[m*n + i] = P_{j i}, j = NL[m][i]
+    void* Q;                // K*n*32 bytes
+    unsigned long long* MASK;  // [n] bit m set <=> slot m is inside the force range
+    // cell structures
+    int64_t cell_cap;
+    int32_t* cell_count;    // [ncell+1] -> exclusive scan in place = cell_start
+    int32_t* cell_of;       // [n]
+    int32_t* rank_in_cell;  // [n]
+    double4* sorted;        // [n] {x,y,z, index bits} in cell order
+    int32_t* scan_blocks;   // block sums scratch
+    // status
+    int* d_status;          // [2]: status bits, max row length seen
+    // e2e device state (md_nve_run_host)
+    double* e2e;            // [13][n] x,y,z,vx,vy,vz,f[3],pe + spare
+    int64_t e2e_cap;
+};
+
+__device__ __forceinline__ double md_min_image(double d, double L, double halfL) {
+    // reading A7: coordinates in [0,L) => |d| < L, one conditional shift
+    if (d > halfL) d -= L;
+    else if (d < -halfL) d += L;
+    return d;
+}
+
+// kernels' launchers (defined in the .cu files)
+int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                    const double box[3], double r_list, cudaStream_t s);
+int md_launch_reverse(md_neighbors* nl, cudaStream_t s);
+int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                      const double* vx, const double* vy, const double* vz, const double box[3],
+                      const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
+                      double* heat, cudaStream_t s);
+int md_launch_sw(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                 const double* vx, const double* vy, const double* vz, const double box[3],
+                 const md_sw_params* p, int precision, double* pe, double* f, double* virial,
+                 double* heat, cudaStream_t s);
+int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                     const double* vx, const double* vy, const double* vz, const double box[3],
+                     int precision, double* f, double* virial, double* heat, cudaStream_t s);
+int md_launch_vv(int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                 const double* f, double mass, double dt, const double box[3], cudaStream_t s);
+int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);

@@ -1,0 +1,79 @@
+// gather.cu -- step C: one thread per atom, no atomics (Algorithm 2 lines 12-17, PAPER.md:278-291;
+// Eqs. 28-30).
+//
+// The pair kernel left in f / virial the "own" halves  sum_j P_ij  and  -1/2 sum_j r_ij (x) P_ij,
+// and pushed P_ji into row i of Q.  Thread i reads its row (coalesced 32-byte records) and finishes
+//   F_i  = sum_j P_ij - sum_j P_ji
+//   W_i  = -1/2 sum_j r_ij (x) P_ij + 1/2 sum_j r_ij (x) P_ji
+//   J_i  = sum_j r_ij (P_ji . v_i)
+#include "common.cuh"
+#include "real_math.cuh"
+
+namespace {
+
+template <class T, class Rec>
+__global__ void __launch_bounds__(256)
+k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+         const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+         double Lx, double Ly, double Lz, const int32_t* __restrict__ NL, const Rec* __restrict__ Q,
+         const unsigned long long* __restrict__ MASK, double* __restrict__ f, double* __restrict__ virial,
+         double* __restrict__ heat) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned long long mask = MASK[i];
+    const bool geom = virial != nullptr || heat != nullptr;
+    double xi = 0, yi = 0, zi = 0;
+    T vxi = T(0), vyi = T(0), vzi = T(0);
+    if (geom) { xi = x[i]; yi = y[i]; zi = z[i]; }
+    if (heat) { vxi = (T)vx[i]; vyi = (T)vy[i]; vzi = (T)vz[i]; }
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    T Jx = T(0), Jy = T(0), Jz = T(0);
+    while (mask) {
+        const int m = __ffsll((long long)mask) - 1;
+        mask &= mask - 1;
+        T px, py, pz;
+        rm::load_rec(&Q[(int64_t)m * n + i], &px, &py, &pz);
+        Fx += px; Fy += py; Fz += pz;
+        if (geom) {
+            const int j = NL[(int64_t)m * n + i];
+            const T rx = (T)md_min_image(x[j] - xi, Lx, 0.5 * Lx);
+            const T ry = (T)md_min_image(y[j] - yi, Ly, 0.5 * Ly);
+            const T rz = (T)md_min_image(z[j] - zi, Lz, 0.5 * Lz);
+            if (virial) {
+                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+            }
+            if (heat) {
+                const T dot = px * vxi + py * vyi + pz * vzi;
+                Jx += rx * dot; Jy += ry * dot; Jz += rz * dot;
+            }
+        }
+    }
+    if (f) {
+        f[i] -= (double)Fx; f[n + i] -= (double)Fy; f[2 * n + i] -= (double)Fz;
+    }
+    if (virial) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] += (double)(T(0.5) * W[q]);
+    }
+    if (heat) { heat[i] = (double)Jx; heat[n + i] = (double)Jy; heat[2 * n + i] = (double)Jz; }
+}
+
+}  // namespace
+
+int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                     const double* vx, const double* vy, const double* vz, const double box[3],
+                     int precision, double* f, double* virial, double* heat, cudaStream_t s) {
+    if (n == 0 || (!f && !virial && !heat)) return MD_OK;
+    const unsigned gb = (unsigned)((n + 255) / 256);
+    if (precision == MD_FP32)
+        k_gather<float, float4><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
+                                                   (const float4*)nl->Q, nl->MASK, f, virial, heat);
+    else
+        k_gather<double, PairRec64><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
+                                                       (const PairRec64*)nl->Q, nl->MASK, f, virial, heat);
+    MD_CUDA_TRY(cudaGetLastError());
+    return MD_OK;
+}

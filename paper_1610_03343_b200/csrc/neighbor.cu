@@ -1,0 +1,237 @@
+// neighbor.cu -- periodic cell-list Verlet neighbour build (A7).
+//
+//   k_bin      cell id per atom + histogram (integer atomics; the force path has none)
+//   k_scan_*   exclusive prefix sum of the histogram with warp-shuffle scans (counting sort)
+//   k_scatter  atoms -> cell order as 32-byte {x,y,z,index} records
+//   k_search   one thread per atom (cell order): 27-cell search, strict d2 < r_list^2,
+//              row sorted by index, neighbour-major store NL[m*n+i]
+//   k_reverse  REV[m*n+i] = position of i in row NL[m*n+i]
+#include "common.cuh"
+
+namespace {
+
+struct Grid {
+    int nc[3];
+    double inv_cell[3];   // nc / L
+    double L[3], halfL[3];
+    double rc2;
+};
+
+__device__ __forceinline__ int cell_coord(double c, double inv, int nc) {
+    int k = (int)(c * inv);
+    k = k < 0 ? 0 : k;
+    return k >= nc ? nc - 1 : k;
+}
+
+__global__ void k_bin(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                      const double* __restrict__ z, Grid g, int32_t* __restrict__ cell_of,
+                      int32_t* __restrict__ rank, int32_t* __restrict__ cell_count) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int cx = cell_coord(x[i], g.inv_cell[0], g.nc[0]);
+    const int cy = cell_coord(y[i], g.inv_cell[1], g.nc[1]);
+    const int cz = cell_coord(z[i], g.inv_cell[2], g.nc[2]);
+    const int c = (cx * g.nc[1] + cy) * g.nc[2] + cz;
+    cell_of[i] = c;
+    rank[i] = atomicAdd(&cell_count[c], 1);
+}
+
+// ---- exclusive scan: tile-local scan, scan of tile totals, add back -------------------------
+constexpr int SCAN_BT = 512;
+constexpr int SCAN_IT = 4;
+
+__device__ __forceinline__ int warp_inclusive_scan(int v) {
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += t;
+    }
+    return v;
+}
+
+// block-wide exclusive scan of one value per thread; returns the exclusive prefix, *total = block sum
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total, int* warp_sums /*[32]*/) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int inc = warp_inclusive_scan(v);
+    if (lane == 31) warp_sums[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        int s = lane < nw ? warp_sums[lane] : 0;
+        s = warp_inclusive_scan(s);
+        warp_sums[lane] = s;
+    }
+    __syncthreads();
+    const int base = wid ? warp_sums[wid - 1] : 0;
+    *total = warp_sums[31];
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void k_scan_local(int32_t* __restrict__ data, int64_t n, int32_t* __restrict__ tile_sums) {
+    __shared__ int warp_sums[32];
+    const int64_t base = ((int64_t)blockIdx.x * SCAN_BT + threadIdx.x) * SCAN_IT;
+    int v[SCAN_IT];
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_IT; ++k) {
+        v[k] = base + k < n ? data[base + k] : 0;
+        s += v[k];
+    }
+    int total;
+    int pre = block_exclusive_scan(s, &total, warp_sums);
+#pragma unroll
+    for (int k = 0; k < SCAN_IT; ++k) {
+        if (base + k < n) data[base + k] = pre;
+        pre += v[k];
+    }
+    if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
+}
+
+__global__ void k_scan_tiles(int32_t* __restrict__ tile_sums, int ntiles) {
+    __shared__ int warp_sums[32];
+    int carry = 0;
+    for (int b = 0; b < ntiles; b += blockDim.x) {
+        const int idx = b + threadIdx.x;
+        const int v = idx < ntiles ? tile_sums[idx] : 0;
+        int total;
+        const int pre = block_exclusive_scan(v, &total, warp_sums);
+        if (idx < ntiles) tile_sums[idx] = carry + pre;
+        carry += total;
+    }
+}
+
+__global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t* __restrict__ tile_sums,
+                           int32_t grand_total) {
+    const int64_t base = ((int64_t)blockIdx.x * SCAN_BT + threadIdx.x) * SCAN_IT;
+    const int add = tile_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_IT; ++k)
+        if (base + k < n) data[base + k] += add;
+    if (blockIdx.x == 0 && threadIdx.x == 0) data[n] = grand_total;
+}
+
+__global__ void k_scatter(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                          const double* __restrict__ z, const int32_t* __restrict__ cell_of,
+                          const int32_t* __restrict__ rank, const int32_t* __restrict__ cell_start,
+                          double4* __restrict__ sorted) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int pos = cell_start[cell_of[i]] + rank[i];
+    sorted[pos] = make_double4(x[i], y[i], z[i], __longlong_as_double((long long)i));
+}
+
+__global__ void __launch_bounds__(128)
+k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const int32_t* __restrict__ cell_of,
+         const int32_t* __restrict__ cell_start, int K, int32_t* __restrict__ NN,
+         int32_t* __restrict__ NL, int* __restrict__ status) {
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const double4 a = sorted[t];
+    const int i = (int)__double_as_longlong(a.w);
+    const int c = cell_of[i];
+    const int cz = c % g.nc[2];
+    const int cy = (c / g.nc[2]) % g.nc[1];
+    const int cx = c / (g.nc[2] * g.nc[1]);
+    int nb[MD_MAX_NEIGHBORS];
+    int cnt = 0;
+    for (int ox = -1; ox <= 1; ++ox) {
+        int ax = cx + ox; ax = ax < 0 ? ax + g.nc[0] : (ax >= g.nc[0] ? ax - g.nc[0] : ax);
+        for (int oy = -1; oy <= 1; ++oy) {
+            int ay = cy + oy; ay = ay < 0 ? ay + g.nc[1] : (ay >= g.nc[1] ? ay - g.nc[1] : ay);
+            for (int oz = -1; oz <= 1; ++oz) {
+                int az = cz + oz; az = az < 0 ? az + g.nc[2] : (az >= g.nc[2] ? az - g.nc[2] : az);
+                const int cc = (ax * g.nc[1] + ay) * g.nc[2] + az;
+                const int beg = cell_start[cc], end = cell_start[cc + 1];
+                for (int q = beg; q < end; ++q) {
+                    const double4 b = sorted[q];
+                    const int j = (int)__double_as_longlong(b.w);
+                    // canonical predicate (reading A7): explicit roundings, no contraction
+                    const double dx = md_min_image(__dsub_rn(b.x, a.x), g.L[0], g.halfL[0]);
+                    const double dy = md_min_image(__dsub_rn(b.y, a.y), g.L[1], g.halfL[1]);
+                    const double dz = md_min_image(__dsub_rn(b.z, a.z), g.L[2], g.halfL[2]);
+                    const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+                    if (d2 < g.rc2 && j != i) {
+                        if (cnt < K) {
+                            int p = cnt;                      // insertion keeps the row sorted by j
+                            while (p > 0 && nb[p - 1] > j) { nb[p] = nb[p - 1]; --p; }
+                            nb[p] = j;
+                        }
+                        ++cnt;
+                    }
+                }
+            }
+        }
+    }
+    atomicMax(&status[1], cnt);
+    if (cnt > K) { atomicOr(&status[0], MD_DEV_ROW_OVERFLOW); cnt = K; }
+    NN[i] = cnt;
+    for (int m = 0; m < cnt; ++m) NL[(int64_t)m * n + i] = nb[m];
+}
+
+__global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                          uint8_t* __restrict__ REV, int* __restrict__ status) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int nn = NN[i];
+    for (int m = 0; m < nn; ++m) {
+        const int j = NL[(int64_t)m * n + i];
+        const int nj = NN[j];
+        int mm = -1;
+        for (int q = 0; q < nj; ++q)
+            if (NL[(int64_t)q * n + j] == (int)i) { mm = q; break; }
+        if (mm < 0) { atomicOr(&status[0], MD_DEV_NO_REVERSE); mm = 0; }
+        REV[(int64_t)m * n + i] = (uint8_t)mm;
+    }
+}
+
+}  // namespace
+
+int md_launch_reverse(md_neighbors* nl, cudaStream_t s) {
+    const int64_t n = nl->n;
+    if (n == 0) return MD_OK;
+    k_reverse<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
+    MD_CUDA_TRY(cudaGetLastError());
+    return MD_OK;
+}
+
+int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                    const double box[3], double r_list, cudaStream_t s) {
+    Grid g;
+    int64_t ncell = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.nc[a] = (int)(box[a] / r_list);
+        if (g.nc[a] < 3) return MD_ERR_BOX_TOO_SMALL;
+        g.inv_cell[a] = (double)g.nc[a] / box[a];
+        g.L[a] = box[a];
+        g.halfL[a] = 0.5 * box[a];
+        ncell *= g.nc[a];
+    }
+    g.rc2 = r_list * r_list;
+    if (ncell + 1 > nl->cell_cap) {                       // grow cell arrays (rare: first build)
+        if (ncell + 1 > (int64_t)2000000000) return MD_ERR_ARG;
+        MD_CUDA_TRY(cudaStreamSynchronize(s));
+        if (nl->cell_count) cudaFree(nl->cell_count);
+        if (nl->scan_blocks) cudaFree(nl->scan_blocks);
+        nl->cell_count = nullptr; nl->scan_blocks = nullptr; nl->cell_cap = 0;
+        const int64_t tiles = (ncell + SCAN_BT * SCAN_IT - 1) / (SCAN_BT * SCAN_IT);
+        if (cudaMalloc(&nl->cell_count, sizeof(int32_t) * (ncell + 1)) != cudaSuccess) return MD_ERR_ALLOC;
+        if (cudaMalloc(&nl->scan_blocks, sizeof(int32_t) * (tiles + 1)) != cudaSuccess) return MD_ERR_ALLOC;
+        nl->cell_cap = ncell + 1;
+    }
+    nl->n = n;
+    if (n == 0) return MD_OK;
+    const int ntiles = (int)((ncell + SCAN_BT * SCAN_IT - 1) / (SCAN_BT * SCAN_IT));
+    const unsigned gb = (unsigned)((n + 255) / 256);
+    MD_CUDA_TRY(cudaMemsetAsync(nl->cell_count, 0, sizeof(int32_t) * (ncell + 1), s));
+    k_bin<<<gb, 256, 0, s>>>(n, x, y, z, g, nl->cell_of, nl->rank_in_cell, nl->cell_count);
+    k_scan_local<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks);
+    k_scan_tiles<<<1, 1024, 0, s>>>(nl->scan_blocks, ntiles);
+    k_scan_add<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks, (int32_t)n);
+    k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted);
+    k_search<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, g, nl->sorted, nl->cell_of, nl->cell_count, nl->K,
+                                                       nl->NN, nl->NL, nl->d_status);
+    MD_CUDA_TRY(cudaGetLastError());
+    return md_launch_reverse(nl, s);
+}

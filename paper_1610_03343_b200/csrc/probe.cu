@@ -1,0 +1,48 @@
+// probe.cu -- FP64 FMA throughput probe: the measured ALU peak the roofline of the (ALU-bound)
+// pair kernels is reported against (MEASURED_PEAKS.json has no FP64 entry).
+#include "common.cuh"
+
+namespace {
+constexpr int CHAINS = 8;
+
+__global__ void __launch_bounds__(256) k_dfma(int iters, double a, double b, double* __restrict__ out) {
+    double v[CHAINS];
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) v[c] = (double)(threadIdx.x + c);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int c = 0; c < CHAINS; ++c) v[c] = __fma_rn(v[c], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) s += v[c];
+    if (s == 123.456) out[0] = s;        // never true; keeps the chains alive
+}
+}  // namespace
+
+int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s) {
+    int dev = 0, sms = 0;
+    MD_CUDA_TRY(cudaGetDevice(&dev));
+    MD_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d_out = nullptr;
+    MD_CUDA_TRY(cudaMalloc(&d_out, sizeof(double)));
+    cudaEvent_t e0, e1;
+    MD_CUDA_TRY(cudaEventCreate(&e0));
+    MD_CUDA_TRY(cudaEventCreate(&e1));
+    const int blocks = sms * 8, threads = 256;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, s);
+        k_dfma<<<blocks, threads, 0, s>>>(iters, 0.999999, 1e-9, d_out);
+        cudaEventRecord(e1, s);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    MD_CUDA_TRY(cudaGetLastError());
+    const double flops = 2.0 * (double)blocks * threads * (double)iters * CHAINS;
+    *tflops = flops / ((double)best * 1e-3) / 1e12;
+    return MD_OK;
+}

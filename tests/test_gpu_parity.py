@@ -1,0 +1,256 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import md_inputs as mi
+import oracle
+import paper_1610_03343_b200 as md
+from gpu_util import (DEV, GpuSystem, assert_close_energy, assert_close_fp32, assert_close_fp64, dev)
+
+pytestmark = pytest.mark.gpu
+PARAMS = {"tersoff": mi.TERSOFF_SI_C, "sw": mi.SW_SI}
+KMAX = {"tersoff": 16, "sw": 32}
+
+CASES = [  # potential, ncell, sigma, T, seed
+    ("tersoff", 2, 0.05, 300.0, 1), ("tersoff", 4, 0.05, 300.0, mi.BASE_SEED), ("tersoff", 5, 0.15, 1500.0, 2),
+    ("tersoff", 7, 0.25, 1500.0, 3), ("sw", 3, 0.05, 300.0, 4), ("sw", 5, 0.15, 1500.0, 5),
+]
+
+
+# ------------------------------------------------------------------ neighbour lists: bit exact
+@pytest.mark.parametrize("pot,ncell,sigma,T,seed", CASES)
+def test_neighbor_list_bit_exact(pot, ncell, sigma, T, seed):
+    s = mi.silicon_crystal(ncell, sigma, T, seed)
+    g = GpuSystem(s, KMAX[pot])
+    mx = g.build(mi.r_list(pot))
+    NN, NL = g.export_list()
+    rNN, rNL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list(pot), KMAX[pot])
+    assert mx == rNN.max()
+    assert (NN == rNN).all()
+    assert (NL == rNL).all()
+
+
+def test_neighbor_list_random_gas_non_cubic_box():
+    rng = np.random.default_rng(12)
+    box = np.array([13.0, 17.5, 22.0])
+    n = 1200
+    P = rng.random((n, 3)) * box
+    s = {"x": P[:, 0].copy(), "y": P[:, 1].copy(), "z": P[:, 2].copy(), "box": box}
+    g = GpuSystem(s, 64)
+    g.build(3.1)
+    NN, NL = g.export_list()
+    rNN, rNL = oracle.neighbors(s["x"], s["y"], s["z"], box, 3.1, 64, method="brute")
+    assert (NN == rNN).all() and (NL == rNL).all()
+    assert NN.min() < NN.max()
+
+
+# ------------------------------------------------------------------ FP64 forces, all outputs
+@pytest.mark.parametrize("pot,ncell,sigma,T,seed", CASES)
+def test_force_virial_heat_energy_fp64(pot, ncell, sigma, T, seed):
+    s = mi.silicon_crystal(ncell, sigma, T, seed)
+    g = GpuSystem(s, KMAX[pot])
+    g.build(mi.r_list(pot))
+    out = g.force(pot, PARAMS[pot])
+    NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list(pot), KMAX[pot])
+    ref = oracle.evaluate(pot, PARAMS[pot], s["x"], s["y"], s["z"], s["box"], NN, NL,
+                          v=(s["vx"], s["vy"], s["vz"]), precision="f80")
+    assert_close_energy(out["pe"], ref["pe"])
+    assert abs(math.fsum(out["pe"]) - math.fsum(ref["pe"])) <= 1e-12 * abs(math.fsum(ref["pe"]))
+    assert_close_fp64("f", out["f"], ref["f"])                 # conventional (Alg. 1) forces
+    assert_close_fp64("virial", out["virial"], ref["virial"])
+    assert_close_fp64("heat", out["heat"], ref["heat"])
+
+
+def test_force_with_imported_oracle_list_and_optional_outputs():
+    s = mi.make_config(0)
+    NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], s["r_list"], 16)
+    g = GpuSystem(s, 16)
+    g.import_list(NN, NL)
+    ref = oracle.evaluate("tersoff", s["params"], s["x"], s["y"], s["z"], s["box"], NN, NL, precision="f80")
+    full = g.force("tersoff", s["params"])
+    only_f = g.force("tersoff", s["params"], want=("f",))
+    only_pe = g.force("tersoff", s["params"], want=("pe",))
+    assert_close_fp64("f", full["f"], ref["f"])
+    assert (only_f["f"] == full["f"]).all()                    # bitwise: outputs do not depend on what is asked
+    assert (only_pe["pe"] == full["pe"]).all()
+
+
+def test_run_to_run_bitwise_reproducible():
+    s = mi.silicon_crystal(6, 0.15, 1500.0, 77)
+    a = GpuSystem(s, 16); a.build(3.5); oa = a.force("tersoff", mi.TERSOFF_SI_C)
+    b = GpuSystem(s, 16); b.build(3.5); ob = b.force("tersoff", mi.TERSOFF_SI_C)
+    for k in oa:
+        assert (oa[k] == ob[k]).all(), k
+
+
+# ------------------------------------------------------------------ FP32 mode
+@pytest.mark.parametrize("pot,ncell,sigma,T,seed", [("tersoff", 5, 0.15, 1500.0, 2), ("sw", 5, 0.05, 300.0, 8)])
+def test_fp32_mode_within_1e4_of_fp64_oracle(pot, ncell, sigma, T, seed):
+    s = mi.silicon_crystal(ncell, sigma, T, seed)
+    g = GpuSystem(s, KMAX[pot])
+    g.build(mi.r_list(pot))
+    out = g.force(pot, PARAMS[pot], precision=md.MD_FP32)
+    NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list(pot), KMAX[pot])
+    ref = oracle.evaluate(pot, PARAMS[pot], s["x"], s["y"], s["z"], s["box"], NN, NL,
+                          v=(s["vx"], s["vy"], s["vz"]))
+    assert np.abs(out["pe"] - ref["pe"]).max() <= 1e-4 * np.abs(ref["pe"]).min()
+    assert abs(out["pe"].sum() - ref["pe"].sum()) <= 1e-4 * abs(ref["pe"].sum())
+    assert_close_fp32("f", out["f"], ref["f"])
+    assert_close_fp32("virial", out["virial"], ref["virial"])
+    assert_close_fp32("heat", out["heat"], ref["heat"])
+
+
+# ------------------------------------------------------------------ degenerate cases
+def test_dimer_and_isolated_atoms_zeta_zero_path():
+    box = np.array([40.0, 40.0, 40.0])
+    for r in (2.0, 2.35, 2.85, 2.95, 3.2):
+        s = {"x": np.array([10.0, 10.0 + r, 30.0]), "y": np.array([10.0, 10.0, 30.0]),
+             "z": np.array([10.0, 10.0, 30.0]), "box": box}
+        g = GpuSystem(s, 16)
+        g.build(3.5)
+        out = g.force("tersoff", mi.TERSOFF_SI_C)
+        NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], box, 3.5, 16)
+        ref = oracle.evaluate("tersoff", mi.TERSOFF_SI_C, s["x"], s["y"], s["z"], box, NN, NL,
+                              v=(np.zeros(3),) * 3, precision="f80")
+        assert np.isfinite(out["f"]).all()
+        assert_close_fp64("pe", out["pe"], ref["pe"], rel=1e-12, floor=1e-15)
+        assert_close_fp64("f", out["f"], ref["f"])
+        assert (out["f"][:, 2] == 0).all() and out["pe"][2] == 0
+
+
+def test_perfect_lattice_zero_force():
+    x, y, z, L = mi.diamond_lattice(4)
+    s = {"x": x, "y": y, "z": z, "box": np.array([L, L, L])}
+    for pot in ("tersoff", "sw"):
+        g = GpuSystem(s, KMAX[pot])
+        mx = g.build(mi.r_list(pot))
+        assert mx == (4 if pot == "tersoff" else 16)
+        out = g.force(pot, PARAMS[pot])
+        assert np.abs(out["f"]).max() <= 1e-12
+
+
+def test_errors_and_empty_input():
+    s = mi.silicon_crystal(2, 0.05, 300.0, 1)
+    g = GpuSystem(s, 16)
+    with pytest.raises(md.MDError) as e:                      # force before any list
+        g.force("tersoff", mi.TERSOFF_SI_C)
+    assert e.value.code == md.MD_ERR_NO_LIST
+    with pytest.raises(md.MDError) as e:                      # 10.86 / 4.0 -> 2 cells
+        md.md_build_neighbors(g.nl, g.n, g.x, g.y, g.z, g.box, 4.0)
+    assert e.value.code == md.MD_ERR_BOX_TOO_SMALL
+    small = GpuSystem(s, 3)                                    # rows of 4 do not fit in K = 3
+    md.md_build_neighbors(small.nl, small.n, small.x, small.y, small.z, small.box, 3.5)
+    assert md.md_neighbors_status(small.nl, check=False) == md.MD_ERR_NEIGHBOR_OVERFLOW
+    with pytest.raises(md.MDError):
+        md.md_neighbors_create(10, 65)
+    # n = 0 is legal everywhere
+    e0 = md.md_neighbors_create(0, 16)
+    z0 = torch.zeros(0, dtype=torch.float64, device=DEV)
+    md.md_build_neighbors(e0, 0, z0, z0, z0, [10.0, 10.0, 10.0], 3.0)
+    md.md_tersoff_force(e0, 0, z0, z0, z0, z0, z0, z0, [10.0, 10.0, 10.0], mi.TERSOFF_SI_C, f=z0)
+    md.md_velocity_verlet_step(0, 0, z0, z0, z0, z0, z0, z0, z0, 28.0, 1.0, [10.0, 10.0, 10.0])
+    assert md.md_neighbors_status(e0) == 0
+
+
+# ------------------------------------------------------------------ integrator and NVE loop
+def test_velocity_verlet_half_steps_match_oracle():
+    s = mi.silicon_crystal(3, 0.05, 300.0, 9)
+    rng = np.random.default_rng(1)
+    f = rng.normal(size=(3, s["n"]))
+    s["x"][:5] = [0.0, 1e-9, s["box"][0] - 1e-12, s["box"][0] * (1 - 2e-16), 5.0]   # wrap edges
+    s["vx"][:5] = [-1e-3, -1.0, 1.0, 1e-3, 0.0]
+    g = GpuSystem(s, 16)
+    fd = dev(f)
+    md.md_velocity_verlet_step(0, g.n, g.x, g.y, g.z, g.vx, g.vy, g.vz, fd, g.mass, 1.0, g.box)
+    ref = {k: s[k].copy() for k in ("x", "y", "z", "vx", "vy", "vz")}
+    oracle.vv_kick_drift(ref["x"], ref["y"], ref["z"], ref["vx"], ref["vy"], ref["vz"], f, s["mass"], 1.0, s["box"])
+    st = g.state()
+    for k in ref:
+        assert np.abs(st[k] - ref[k]).max() <= 1e-13 * max(1.0, np.abs(ref[k]).max()), k
+    for k in "xyz":
+        assert (st[k] >= 0).all() and (st[k] < s["box"][0]).all()
+    md.md_velocity_verlet_step(1, g.n, g.x, g.y, g.z, g.vx, g.vy, g.vz, fd, g.mass, 1.0, g.box)
+    oracle.vv_kick(ref["vx"], ref["vy"], ref["vz"], f, s["mass"], 1.0)
+    st = g.state()
+    for k in ("vx", "vy", "vz"):
+        assert np.abs(st[k] - ref[k]).max() <= 1e-15
+
+
+@pytest.mark.parametrize("pot", ["tersoff", "sw"])
+def test_nve_run_short_trajectory_and_snapshot_parity(pot):
+    """25 steps stay within rounding-amplified distance of the oracle trajectory; then snapshot parity:
+    the GPU state is handed to the oracle and one evaluation is compared at full tolerance."""
+    s = mi.silicon_crystal(3, 0.05, 300.0, 15)
+    K = KMAX[pot]
+    g = GpuSystem(s, K)
+    n = g.n
+    f = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+    pe = torch.zeros(n, dtype=torch.float64, device=DEV)
+    md.md_nve_run(g.nl, pot, PARAMS[pot], n, g.x, g.y, g.z, g.vx, g.vy, g.vz, f, False, pe, g.box, g.mass,
+                  1.0, 25, 10, mi.r_list(pot))
+    md.md_neighbors_status(g.nl)
+    ref = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in s.items()}
+    r = oracle.nve_run(pot, PARAMS[pot], ref, 25, 1.0, 10, mi.r_list(pot), K)
+    st = g.state()
+    for k in ("x", "y", "z"):
+        d = np.abs(st[k] - ref[k]); d = np.minimum(d, s["box"][0] - d)
+        assert d.max() <= 1e-9, k
+    for k in ("vx", "vy", "vz"):
+        assert np.abs(st[k] - ref[k]).max() <= 1e-11, k
+    # snapshot parity on the GPU's own final state (list of step 20, as the GPU used it)
+    NN, NL = g.export_list()
+    snap = oracle.evaluate(pot, PARAMS[pot], st["x"], st["y"], st["z"], st["box"], NN, NL, precision="f80")
+    assert_close_fp64("f", f.cpu().numpy(), snap["f"])
+    assert_close_energy(pe.cpu().numpy(), snap["pe"])
+    assert abs(math.fsum(r["pe"]) - math.fsum(snap["pe"])) <= 1e-9 * abs(math.fsum(snap["pe"]))
+
+
+@pytest.mark.parametrize("pot", ["tersoff", "sw"])
+def test_nve_energy_conservation_on_gpu(pot):
+    s = mi.silicon_crystal(4, 0.05, 300.0, 19)
+    K = KMAX[pot]
+    dev_e = []
+    for dt, nsteps in ((1.0, 100), (0.5, 200)):
+        g = GpuSystem(s, K)
+        n = g.n
+        f = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+        pe = torch.zeros(n, dtype=torch.float64, device=DEV)
+
+        def total():
+            ke = 0.5 * g.mass * float((g.vx ** 2 + g.vy ** 2 + g.vz ** 2).sum()) / mi.KAPPA
+            return ke + float(pe.sum())
+        md.md_nve_run(g.nl, pot, PARAMS[pot], n, g.x, g.y, g.z, g.vx, g.vy, g.vz, f, False, pe, g.box, g.mass,
+                      dt, 0, 10, mi.r_list(pot))
+        e0 = total()
+        worst = 0.0
+        for _ in range(nsteps // 10):
+            md.md_nve_run(g.nl, pot, PARAMS[pot], n, g.x, g.y, g.z, g.vx, g.vy, g.vz, f, True, pe, g.box, g.mass,
+                          dt, 10, 10, mi.r_list(pot))
+            worst = max(worst, abs(total() - e0) / n)
+        md.md_neighbors_status(g.nl)
+        dev_e.append(worst)
+    assert dev_e[0] <= 1e-4, dev_e
+    assert 3.0 <= dev_e[0] / dev_e[1] <= 5.0, dev_e
+
+
+def test_nve_run_host_matches_device_run():
+    s = mi.silicon_crystal(3, 0.05, 300.0, 15)
+    g = GpuSystem(s, 16)
+    n = g.n
+    f = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+    pe = torch.zeros(n, dtype=torch.float64, device=DEV)
+    md.md_nve_run(g.nl, "tersoff", mi.TERSOFF_SI_C, n, g.x, g.y, g.z, g.vx, g.vy, g.vz, f, False, pe, g.box,
+                  g.mass, 1.0, 12, 10, 3.5)
+    h = {k: torch.from_numpy(s[k].copy()).pin_memory() for k in ("x", "y", "z", "vx", "vy", "vz")}
+    hf = torch.zeros((3, n), dtype=torch.float64).pin_memory()
+    hpe = torch.zeros(n, dtype=torch.float64).pin_memory()
+    nl2 = md.md_neighbors_create(n, 16)
+    md.md_nve_run_host(nl2, "tersoff", mi.TERSOFF_SI_C, n, h["x"], h["y"], h["z"], h["vx"], h["vy"], h["vz"],
+                       hf, hpe, g.box, g.mass, 1.0, 12, 10, 3.5)
+    st = g.state()
+    for k in h:
+        assert (h[k].numpy() == st[k]).all(), k
+    assert (hf.numpy() == f.cpu().numpy()).all() and (hpe.numpy() == pe.cpu().numpy()).all()
