@@ -104,14 +104,14 @@ int md_velocity_verlet_step(int phase, int64_t n, double* x, double* y, double* 
                             double mass_amu, double dt_fs, const double box[3], void* stream);
 
 /* Convenience: nsteps NVE steps composed of the four calls above, list rebuilt after the drift of
- * every step s with s % rebuild_every == 0.  `params` is a HOST md_tersoff_params* or md_sw_params*
+ * every step s (counted from first_step) with s % rebuild_every == 0.  `params` is a HOST md_tersoff_params* or md_sw_params*
  * according to `potential`.  f[3][n] must hold the forces of the incoming state if f_valid != 0,
  * otherwise they are computed first (with a list built at the incoming positions).
  * pe[n] (may be NULL) receives U_i of the final state. */
 int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                double* x, double* y, double* z, double* vx, double* vy, double* vz,
                double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
-               int nsteps, int rebuild_every, double r_list, void* stream);
+               int first_step, int nsteps, int rebuild_every, double r_list, void* stream);
 
 /* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
  * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
@@ -125,6 +125,15 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
  * full grid and returns the achieved FP64 rate in *tflops (HOST); used as the measured ALU peak of
  * the roofline.  Synchronous. */
 int md_probe_fp64_peak(int iters, double* tflops, void* stream);
+
+/* Per-kernel-kind device timing (CUDA events on the launching stream) and launch counts.
+ * md_profile_enable(nl, 1) starts recording an event pair around every kernel group launched
+ * through `nl`; md_profile_read synchronises the device, adds up the elapsed times and resets.
+ * kinds: 0 neighbour build, 1 pair kernel, 2 gather kernel, 3 integrator.  ms[4], launches[4] HOST.
+ * Launch counts (kernels enqueued) are kept whether or not timing is enabled. */
+enum { MD_KIND_BUILD = 0, MD_KIND_PAIR = 1, MD_KIND_GATHER = 2, MD_KIND_INTEGRATE = 3, MD_N_KINDS = 4 };
+int md_profile_enable(md_neighbors* nl, int enable);
+int md_profile_read(md_neighbors* nl, double* ms, int64_t* launches);
 
 /* Library version string (HOST, static storage). */
 const char* md_version(void);

@@ -38,7 +38,8 @@ class md_sw_params(C.Structure):
 
 EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neighbors_status",
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
-           "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak")
+           "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
+           "md_profile_enable", "md_profile_read")
 
 _lib = None
 
@@ -188,13 +189,13 @@ def _pot(potential, params):
 
 
 def md_nve_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, pe, box, mass_amu, dt_fs,
-               nsteps, rebuild_every, r_list, precision=MD_FP64, stream=None):
+               nsteps, rebuild_every, r_list, precision=MD_FP64, stream=None, first_step=0):
     pid, p = _pot(potential, params)
     _check(load().md_nve_run(nl._h, C.c_int(pid), C.byref(p), C.c_int(precision), C.c_int64(n),
                              _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy), _ptr(vz), _ptr(f),
                              C.c_int(1 if f_valid else 0), _ptr(pe), _box(box), C.c_double(mass_amu),
-                             C.c_double(dt_fs), C.c_int(nsteps), C.c_int(rebuild_every), C.c_double(r_list),
-                             _stream(stream)), "md_nve_run")
+                             C.c_double(dt_fs), C.c_int(first_step), C.c_int(nsteps), C.c_int(rebuild_every),
+                             C.c_double(r_list), _stream(stream)), "md_nve_run")
 
 
 def md_nve_run_host(nl, potential, params, n, x, y, z, vx, vy, vz, f, pe, box, mass_amu, dt_fs,
@@ -211,3 +212,18 @@ def md_probe_fp64_peak(iters=20000, stream=None) -> float:
     t = C.c_double(0.0)
     _check(load().md_probe_fp64_peak(C.c_int(iters), C.byref(t), _stream(stream)), "md_probe_fp64_peak")
     return t.value
+
+
+KINDS = ("build", "pair", "gather", "integrate")
+
+
+def md_profile_enable(nl, enable=True):
+    _check(load().md_profile_enable(nl._h, C.c_int(1 if enable else 0)), "md_profile_enable")
+
+
+def md_profile_read(nl):
+    """Synchronises; returns ({kind: ms}, {kind: kernel launches}) since the last read."""
+    ms = (C.c_double * 4)()
+    ln = (C.c_int64 * 4)()
+    _check(load().md_profile_read(nl._h, ms, ln), "md_profile_read")
+    return {k: ms[i] for i, k in enumerate(KINDS)}, {k: int(ln[i]) for i, k in enumerate(KINDS)}

@@ -12,6 +12,8 @@ void free_all(md_neighbors* nl) {
     cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e);
+    if (nl->ev_pool) for (cudaEvent_t e : *nl->ev_pool) cudaEventDestroy(e);
+    delete nl->ev_pool; delete nl->ev_kind;
 }
 
 int force_dispatch(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
@@ -38,7 +40,58 @@ int check_force_args(md_neighbors* nl, int64_t n, const double* x, const double*
 
 }  // namespace
 
+// ---- per-kind launch counting and event timing --------------------------------------------------
+ProfScope::ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_) : nl(nl_), s(s_), e1(nullptr), on(false) {
+    if (!nl) return;
+    nl->launches[kind] += nk;
+    if (!nl->prof_on || !nl->ev_pool) return;
+    while (nl->ev_pool->size() < nl->ev_used + 2) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        nl->ev_pool->push_back(e);
+    }
+    cudaEvent_t e0 = (*nl->ev_pool)[nl->ev_used];
+    e1 = (*nl->ev_pool)[nl->ev_used + 1];
+    nl->ev_used += 2;
+    nl->ev_kind->push_back(kind);
+    cudaEventRecord(e0, s);
+    on = true;
+}
+ProfScope::~ProfScope() { if (on) cudaEventRecord(e1, s); }
+
 extern "C" {
+
+int md_profile_enable(md_neighbors* nl, int enable) {
+    if (!nl) return MD_ERR_ARG;
+    if (enable && !nl->ev_pool) {
+        nl->ev_pool = new (std::nothrow) std::vector<cudaEvent_t>();
+        nl->ev_kind = new (std::nothrow) std::vector<int>();
+        if (!nl->ev_pool || !nl->ev_kind) return MD_ERR_ALLOC;
+    }
+    nl->prof_on = enable ? 1 : 0;
+    return MD_OK;
+}
+
+int md_profile_read(md_neighbors* nl, double* ms, int64_t* launches) {
+    if (!nl) return MD_ERR_ARG;
+    MD_CUDA_TRY(cudaDeviceSynchronize());
+    for (int k = 0; k < MD_N_KINDS; ++k) nl->ms_acc[k] = 0.0;
+    if (nl->ev_pool && nl->ev_kind) {
+        for (size_t q = 0; q < nl->ev_kind->size(); ++q) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, (*nl->ev_pool)[2 * q], (*nl->ev_pool)[2 * q + 1]) == cudaSuccess)
+                nl->ms_acc[(*nl->ev_kind)[q]] += (double)t;
+        }
+        nl->ev_kind->clear();
+        nl->ev_used = 0;
+    }
+    for (int k = 0; k < MD_N_KINDS; ++k) {
+        if (ms) ms[k] = nl->ms_acc[k];
+        if (launches) launches[k] = nl->launches[k];
+        nl->launches[k] = 0;
+    }
+    return MD_OK;
+}
 
 const char* md_version(void) { return "paper_1610_03343_b200 0.1 (sm_100a)"; }
 
@@ -143,14 +196,15 @@ int md_velocity_verlet_step(int phase, int64_t n, double* x, double* y, double* 
     if ((phase != 0 && phase != 1) || n < 0 || !(mass_amu > 0)) return MD_ERR_ARG;
     if (n > 0 && (!vx || !vy || !vz || !f)) return MD_ERR_ARG;
     if (phase == 0 && (!valid_box(box) || (n > 0 && (!x || !y || !z)))) return MD_ERR_ARG;
-    return md_launch_vv(phase, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, (cudaStream_t)stream);
+    return md_launch_vv(nullptr, phase, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, (cudaStream_t)stream);
 }
 
 int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                double* x, double* y, double* z, double* vx, double* vy, double* vz,
                double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
-               int nsteps, int rebuild_every, double r_list, void* stream) {
-    if (!nl || !params || n < 0 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1)
+               int first_step, int nsteps, int rebuild_every, double r_list, void* stream) {
+    if (!nl || !params || n < 0 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1 ||
+        first_step < 0)
         return MD_ERR_ARG;
     if (potential != MD_TERSOFF && potential != MD_SW) return MD_ERR_ARG;
     if (precision != MD_FP64 && precision != MD_FP32) return MD_ERR_ARG;
@@ -163,15 +217,15 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  pe, f, nullptr, nullptr, s)) != MD_OK) return rc;
     }
-    for (int step = 0; step < nsteps; ++step) {
-        if ((rc = md_launch_vv(0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+    for (int step = first_step; step < first_step + nsteps; ++step) {
+        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
         if (step % rebuild_every == 0)
             if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if (nl->n != n) return MD_ERR_NO_LIST;
-        const bool last = step == nsteps - 1;
+        const bool last = step == first_step + nsteps - 1;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  last ? pe : nullptr, f, nullptr, nullptr, s)) != MD_OK) return rc;
-        if ((rc = md_launch_vv(1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
     }
     return MD_OK;
 }
@@ -199,7 +253,7 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
     for (int a = 0; a < 6; ++a)
         MD_CUDA_TRY(cudaMemcpyAsync(d + a * n, host_in[a], bytes, cudaMemcpyHostToDevice, s));
     int rc = md_nve_run(nl, potential, params, precision, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n,
-                        d + 6 * n, 0, d + 9 * n, box, mass_amu, dt_fs, nsteps, rebuild_every, r_list, stream);
+                        d + 6 * n, 0, d + 9 * n, box, mass_amu, dt_fs, 0, nsteps, rebuild_every, r_list, stream);
     if (rc != MD_OK) return rc;
     for (int a = 0; a < 6; ++a)
         MD_CUDA_TRY(cudaMemcpyAsync(host_in[a], d + a * n, bytes, cudaMemcpyDeviceToHost, s));

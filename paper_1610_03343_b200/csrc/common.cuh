@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "md.h"
 
 #define MD_CUDA_TRY(expr)                         \
@@ -44,6 +46,13 @@ struct md_neighbors {
     int32_t* scan_blocks;   // block sums scratch
     // status
     int* d_status;          // [2]: status bits, max row length seen
+    // profiling (md_profile_*)
+    int prof_on;
+    int64_t launches[MD_N_KINDS];
+    std::vector<cudaEvent_t>* ev_pool;                 // all events ever created (reused)
+    std::vector<int>* ev_kind;                         // kind of each recorded pair
+    size_t ev_used;                                    // events handed out since the last read
+    double ms_acc[MD_N_KINDS];
     // e2e device state (md_nve_run_host)
     double* e2e;            // [13][n] x,y,z,vx,vy,vz,f[3],pe + spare
     int64_t e2e_cap;
@@ -55,6 +64,13 @@ __device__ __forceinline__ double md_min_image(double d, double L, double halfL)
     else if (d < -halfL) d += L;
     return d;
 }
+
+// RAII scope: counts `nk` kernel launches of `kind` and, if profiling is on, brackets them with events.
+struct ProfScope {
+    md_neighbors* nl; cudaStream_t s; cudaEvent_t e1; bool on;
+    ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_);
+    ~ProfScope();
+};
 
 // kernels' launchers (defined in the .cu files)
 int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
@@ -71,6 +87,6 @@ int md_launch_sw(md_neighbors* nl, int64_t n, const double* x, const double* y, 
 int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                      const double* vx, const double* vy, const double* vz, const double box[3],
                      int precision, double* f, double* virial, double* heat, cudaStream_t s);
-int md_launch_vv(int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
+int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s);
 int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);

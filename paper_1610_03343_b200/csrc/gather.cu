@@ -68,6 +68,7 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
                      int precision, double* f, double* virial, double* heat, cudaStream_t s) {
     if (n == 0 || (!f && !virial && !heat)) return MD_OK;
     const unsigned gb = (unsigned)((n + 255) / 256);
+    ProfScope prof(nl, MD_KIND_GATHER, 1, s);
     if (precision == MD_FP32)
         k_gather<float, float4><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
                                                    (const float4*)nl->Q, nl->MASK, f, virial, heat);

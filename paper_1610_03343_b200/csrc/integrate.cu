@@ -31,11 +31,12 @@ __global__ void k_kick(int64_t n, double* __restrict__ vx, double* __restrict__ 
 }
 }  // namespace
 
-int md_launch_vv(int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
+int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s) {
     if (n == 0) return MD_OK;
     const double hk = 0.5 * dt * KAPPA / mass;
     const unsigned gb = (unsigned)((n + 255) / 256);
+    ProfScope prof(nl, MD_KIND_INTEGRATE, 1, s);
     if (phase == 0) k_kick_drift<<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, f, hk, dt, box[0], box[1], box[2]);
     else k_kick<<<gb, 256, 0, s>>>(n, vx, vy, vz, f, hk);
     MD_CUDA_TRY(cudaGetLastError());

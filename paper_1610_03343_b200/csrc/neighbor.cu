@@ -191,6 +191,7 @@ __global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, cons
 int md_launch_reverse(md_neighbors* nl, cudaStream_t s) {
     const int64_t n = nl->n;
     if (n == 0) return MD_OK;
+    ProfScope prof(nl, MD_KIND_BUILD, 1, s);
     k_reverse<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
@@ -224,6 +225,8 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     if (n == 0) return MD_OK;
     const int ntiles = (int)((ncell + SCAN_BT * SCAN_IT - 1) / (SCAN_BT * SCAN_IT));
     const unsigned gb = (unsigned)((n + 255) / 256);
+    {
+    ProfScope prof(nl, MD_KIND_BUILD, 6, s);
     MD_CUDA_TRY(cudaMemsetAsync(nl->cell_count, 0, sizeof(int32_t) * (ncell + 1), s));
     k_bin<<<gb, 256, 0, s>>>(n, x, y, z, g, nl->cell_of, nl->rank_in_cell, nl->cell_count);
     k_scan_local<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks);
@@ -232,6 +235,7 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted);
     k_search<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, g, nl->sorted, nl->cell_of, nl->cell_count, nl->K,
                                                        nl->NN, nl->NL, nl->d_status);
+    }
     MD_CUDA_TRY(cudaGetLastError());
     return md_launch_reverse(nl, s);
 }

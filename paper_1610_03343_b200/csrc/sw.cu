@@ -133,6 +133,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.rc = (T)rc; p.rc2 = (T)(rc * rc); p.gs = (T)(hp->gamma * hp->sigma);
     p.leps = (T)(hp->lambda * hp->epsilon); p.cos0 = (T)hp->cos0; p.p = (T)hp->p; p.q = (T)hp->q;
     p.ip = small_int(hp->p); p.iq = small_int(hp->q);
+    ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     k_sw_pair<T, Rec><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(
         n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
         pe, f, virial, nl->d_status);

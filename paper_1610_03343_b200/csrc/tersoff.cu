@@ -156,6 +156,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.c2 = (T)(hp->c * hp->c); p.d2 = (T)(hp->d * hp->d); p.c2_over_d2 = (T)((hp->c * hp->c) / (hp->d * hp->d));
     p.w = (T)(3.14159265358979323846 / (hp->S - hp->R));
     p.minus_half_over_n = (T)(-0.5 / hp->n);
+    ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     k_tersoff_pair<T, Rec><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(
         n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
         pe, f, virial, nl->d_status);
