@@ -86,7 +86,7 @@ def assert_close_energy(got, ref, rel=1e-12):
 
 
 def assert_close_fp32(name, got, ref, rel=1e-4):
-    """DESIGN.md A10: ||d||_2 <= rel ||ref||_2 and max_i |d_i| <= rel * RMS_i |ref_i| * sqrt(3)-free form."""
+    """DESIGN.md A10: ||d||_2 <= rel ||ref||_2 and per-atom |d_i| <= 10 rel * RMS_k |ref_k|."""
     d = got - ref
     assert np.linalg.norm(d) <= rel * np.linalg.norm(ref), (name, np.linalg.norm(d) / np.linalg.norm(ref))
     per_atom = np.sqrt((d ** 2).sum(axis=0))
