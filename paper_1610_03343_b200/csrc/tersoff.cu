@@ -7,8 +7,11 @@
 //     (Q[rev(i,m)*n + j]; exactly one writer per slot, no atomics),
 //   * accumulates the "own" halves  sum_j P_ij  and  -1/2 sum_j r_ij (x) P_ij  and U_i.
 // T = double (MD_FP64) or float (MD_FP32: r_ij formed in double, then rounded; reading A10).
+#include <cstdlib>
+
 #include "common.cuh"
 #include "real_math.cuh"
+#include "pair_cta.cuh"
 
 namespace {
 
@@ -20,19 +23,20 @@ struct TersoffDev {
     T minus_half_over_n;      // -1/(2n)
 };
 
-constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom
+constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom (generic path)
+constexpr int TERSOFF_MR = 6;    // list-row length handled by the register path
 
+// Generic path: any number of in-range neighbours up to TERSOFF_KC, per-thread arrays in local memory.
+// Used by threads whose list row is longer than the register path's MR slots.
 template <class T, class Rec>
-__global__ void __launch_bounds__(128)
-k_tersoff_pair(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+__device__ __noinline__ void
+tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                const double* __restrict__ z, double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                const uint8_t* __restrict__ REV, TersoffDev<T> p,
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                int* __restrict__ status) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
     const double xi = x[i], yi = y[i], zi = z[i];
     const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
     const int nn = NN[i];
@@ -146,6 +150,288 @@ k_tersoff_pair(int64_t n, const double* __restrict__ x, const double* __restrict
     }
 }
 
+// 1/a by MUFU.RCP64H + two Newton steps (4 DFMA): full double accuracy for normal a, no IEEE special cases.
+__device__ __forceinline__ double fast_rcp(double a) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double e = __fma_rn(-a, y, 1.0);
+    y = __fma_rn(y, e, y);
+    e = __fma_rn(-a, y, 1.0);
+    return __fma_rn(y, e, y);
+}
+__device__ __forceinline__ float fast_rcp(float a) { return __frcp_rn(a); }
+
+// Register path: list rows of up to MR entries, every per-neighbour quantity in registers (all array
+// indices are compile-time constants after unrolling; slots m >= nn are skipped by warp-uniform branches).
+// A listed neighbour outside the force range keeps f_C = f_C' = f_R = f_A = 0, so it drops out of every sum.
+template <class T, class Rec, int MR>
+__global__ void __launch_bounds__(128)
+k_tersoff_pair(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+               const double* __restrict__ z, double Lx, double Ly, double Lz,
+               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+               const uint8_t* __restrict__ REV, TersoffDev<T> p,
+               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+               int* __restrict__ status) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int nn = NN[i];
+    if (nn > MR) {
+        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, virial, status);
+        return;
+    }
+    const double xi = x[i], yi = y[i], zi = z[i];
+    const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
+
+    int jd[MR];
+    double dx[MR], dy[MR], dz[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) jd[m] = m < nn ? NL[(int64_t)m * n + i] : (int)i;
+#pragma unroll
+    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
+
+    T ex[MR], ey[MR], ez[MR], rinv[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
+    unsigned mask = 0u;
+#pragma unroll
+    for (int m = 0; m < MR; ++m) {
+        ex[m] = ey[m] = ez[m] = rinv[m] = fc[m] = fcp[m] = fR[m] = fA[m] = zeta[m] = T(0);
+        if (m < nn) {
+            const T tx = (T)md_min_image(dx[m] - xi, Lx, hx);
+            const T ty = (T)md_min_image(dy[m] - yi, Ly, hy);
+            const T tz = (T)md_min_image(dz[m] - zi, Lz, hz);
+            const T d2 = tx * tx + ty * ty + tz * tz;
+            const T ri = rm::rsqrt(d2);
+            const T rr = d2 * ri;
+            ex[m] = tx * ri; ey[m] = ty * ri; ez[m] = tz * ri; rinv[m] = ri;
+            if (d2 < p.S2) {
+                mask |= 1u << m;
+                T c = T(1), cp = T(0);
+                if (rr > p.R) {                              // f_C window R < r < S (reading A1)
+                    T sn, cs;
+                    rm::sincos((rr - p.R) * p.w, &sn, &cs);
+                    c = T(0.5) + T(0.5) * cs;
+                    cp = T(-0.5) * p.w * sn;
+                }
+                fc[m] = c; fcp[m] = cp;
+                fR[m] = p.A * rm::exp(-p.lambda * rr);
+                fA[m] = p.B * rm::exp(-p.mu * rr);
+            }
+        }
+    }
+
+    // zeta (Eq. 4), unordered neighbour pairs visited once (g_ijk = g_ikj for one element)
+#pragma unroll
+    for (int a = 0; a < MR; ++a)
+#pragma unroll
+        for (int b = a + 1; b < MR; ++b)
+            if (b < nn) {
+                const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+                const T xx = p.h - cs;
+                const T x2 = xx * xx;
+                const T g = T(1) + p.c2_over_d2 * x2 * fast_rcp(p.d2 + x2);
+                zeta[a] += fc[b] * g;
+                zeta[b] += fc[a] * g;
+            }
+
+    T U = T(0);
+    T Px[MR], Py[MR], Pz[MR], hh[MR];
+#pragma unroll
+    for (int a = 0; a < MR; ++a) {
+        Px[a] = Py[a] = Pz[a] = hh[a] = T(0);
+        if (a < nn && (mask >> a & 1u)) {
+            T b = T(1), bp = T(0);
+            const T zt = zeta[a];
+            if (zt > T(0)) {                                 // zeta = 0: b = 1, b' = 0 (reading A8)
+                const T t = rm::exp(p.n * rm::log(p.beta * zt));
+                b = rm::exp(p.minus_half_over_n * rm::log1p(t));
+                bp = T(-0.5) * b * t * fast_rcp(zt * (T(1) + t));
+            }
+            const T bfA = b * fA[a];
+            U += T(0.5) * fc[a] * (fR[a] - bfA);
+            const T D = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
+            hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
+            Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
+        }
+    }
+
+#pragma unroll
+    for (int a = 0; a < MR; ++a)
+#pragma unroll
+        for (int b = a + 1; b < MR; ++b)
+            if (b < nn) {
+                const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+                const T xx = p.h - cs;
+                const T x2 = xx * xx;
+                const T q = fast_rcp(p.d2 + x2);
+                const T g = T(1) + p.c2_over_d2 * x2 * q;
+                const T gp = T(-2) * p.c2 * xx * q * q;      // dg/dcos
+                const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
+                const T ta = tab * rinv[a], tb = tab * rinv[b];
+                const T ua = hh[b] * fcp[a] * g - ta * cs;
+                const T ub = hh[a] * fcp[b] * g - tb * cs;
+                Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
+                Px[b] += tb * ex[a] + ub * ex[b]; Py[b] += tb * ey[a] + ub * ey[b]; Pz[b] += tb * ez[a] + ub * ez[b];
+            }
+
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+#pragma unroll
+    for (int a = 0; a < MR; ++a)
+        if (a < nn && (mask >> a & 1u)) {
+            const int mm = REV[(int64_t)a * n + i];
+            rm::store_rec(&Q[(int64_t)mm * n + jd[a]], Px[a], Py[a], Pz[a]);
+            Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
+            if (virial) {
+                const T rr = T(1) / rinv[a];
+                const T rx = ex[a] * rr, ry = ey[a] * rr, rz = ez[a] * rr;
+                W[0] += rx * Px[a]; W[1] += rx * Py[a]; W[2] += rx * Pz[a];
+                W[3] += ry * Px[a]; W[4] += ry * Py[a]; W[5] += ry * Pz[a];
+                W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
+            }
+        }
+    MASK[i] = (unsigned long long)mask;
+    if (pe) pe[i] = (double)U;
+    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+    if (virial) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// "lanes = pairs" kernel (default).  CTA of 256 threads owns TA atoms; one thread per in-range pair.
+//   stage A  compaction of the in-range pairs into shared memory            (pair_cta.cuh)
+//   stage B  per pair: e_ij, 1/r, f_C, f_C', f_R, f_A
+//   stage C  per pair: zeta_ij over the other pairs of the same atom, b_ij, b'_ij, U_ij/2, D, h
+//   stage D  per pair: P_ij (T5), pushed to Q[rev(i,m)*n + j]
+//   stage E  per atom: U_i, own halves sum_j P_ij and -1/2 sum_j r_ij (x) P_ij, MASK
+template <class T, int TA, int PC>
+struct TersoffSmem {
+    pc::Dense<T, TA, PC> d;
+    T rinv[PC], fc[PC], fcp[PC], fRD[PC], fAu[PC], hh[PC];   // fRD: f_R then D; fAu: f_A then U_ij/2
+    T Px[PC], Py[PC], Pz[PC];
+};
+
+template <class T, class Rec, int TA, int PC>
+__global__ void __launch_bounds__(pc::NT)
+k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
+                    const double* __restrict__ z, double Lx, double Ly, double Lz,
+                    const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                    const uint8_t* __restrict__ REV, TersoffDev<T> p,
+                    Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+                    double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+                    int* __restrict__ status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TersoffSmem<T, TA, PC>& s = *reinterpret_cast<TersoffSmem<T, TA, PC>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int64_t A0 = (int64_t)blockIdx.x * TA;
+    const int na = (int)min((int64_t)TA, n - A0);
+    pc::compact_in_range<T, TA, PC>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.S2, status);
+    const int np = s.d.np;
+
+    // stage B
+    for (int k = tid; k < np; k += pc::NT) {
+        const T tx = s.d.ex[k], ty = s.d.ey[k], tz = s.d.ez[k];
+        const T d2 = tx * tx + ty * ty + tz * tz;
+        const T ri = rm::rsqrt(d2);
+        const T rr = d2 * ri;
+        s.d.ex[k] = tx * ri; s.d.ey[k] = ty * ri; s.d.ez[k] = tz * ri; s.rinv[k] = ri;
+        T c = T(1), cp = T(0);
+        if (rr > p.R) {                                      // f_C window R < r < S (reading A1)
+            T sn, cs;
+            rm::sincos((rr - p.R) * p.w, &sn, &cs);
+            c = T(0.5) + T(0.5) * cs;
+            cp = T(-0.5) * p.w * sn;
+        }
+        s.fc[k] = c; s.fcp[k] = cp;
+        s.fRD[k] = p.A * rm::exp(-p.lambda * rr);
+        s.fAu[k] = p.B * rm::exp(-p.mu * rr);
+    }
+    __syncthreads();
+
+    // stage C: zeta_ij = sum_{k != j} f_C(r_ik) g_ijk (Eq. 4); g in the cancellation-free form
+    for (int k = tid; k < np; k += pc::NT) {
+        const int t = s.d.tm[k] >> 6;
+        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
+        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
+        T zt = T(0);
+        for (int b = b0; b < b1; ++b) {
+            if (b == k) continue;
+            const T cs = ax * s.d.ex[b] + ay * s.d.ey[b] + az * s.d.ez[b];
+            const T xx = p.h - cs;
+            const T x2 = xx * xx;
+            zt += s.fc[b] * (T(1) + p.c2_over_d2 * x2 * pc::fast_rcp(p.d2 + x2));
+        }
+        T bo = T(1), bp = T(0);
+        if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
+            const T tt = rm::exp(p.n * rm::log(p.beta * zt));           // (beta zeta)^n
+            bo = rm::exp(p.minus_half_over_n * rm::log1p(tt));          // Eq. (3)
+            bp = T(-0.5) * bo * tt * pc::fast_rcp(zt * (T(1) + tt));
+        }
+        const T c = s.fc[k], cp = s.fcp[k], fR = s.fRD[k], fA = s.fAu[k];
+        const T bfA = bo * fA;
+        s.fAu[k] = T(0.5) * c * (fR - bfA);                                            // U_ij / 2
+        s.fRD[k] = T(0.5) * (cp * (fR - bfA) + c * (p.mu * bfA - p.lambda * fR));      // D
+        s.hh[k] = T(-0.5) * c * fA * bp;                                               // h
+    }
+    __syncthreads();
+
+    // stage D: P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g' (e_b - cos e_a)/r_a + h_b fc'_a g e_a ]
+    for (int k = tid; k < np; k += pc::NT) {
+        const int tmk = s.d.tm[k];
+        const int t = tmk >> 6, m = tmk & 63;
+        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
+        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
+        const T ha = s.hh[k], ca = s.fc[k], cpa = s.fcp[k], ria = s.rinv[k];
+        T ce = s.fRD[k];                                     // coefficient of e_a
+        T sx = T(0), sy = T(0), sz = T(0);                   // sum of ta * e_b
+        for (int b = b0; b < b1; ++b) {
+            if (b == k) continue;
+            const T bx = s.d.ex[b], by = s.d.ey[b], bz = s.d.ez[b];
+            const T cs = ax * bx + ay * by + az * bz;
+            const T xx = p.h - cs;
+            const T x2 = xx * xx;
+            const T q = pc::fast_rcp(p.d2 + x2);
+            const T hb = s.hh[b];
+            const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
+            const T ta = (ha * s.fc[b] + hb * ca) * gp * ria;
+            ce += hb * cpa * (T(1) + p.c2_over_d2 * x2 * q) - ta * cs;
+            sx += ta * bx; sy += ta * by; sz += ta * bz;
+        }
+        const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
+        s.Px[k] = px; s.Py[k] = py; s.Pz[k] = pz;
+        const int64_t i = A0 + t;
+        const int mm = REV[(int64_t)m * n + i];
+        rm::store_rec(&Q[(int64_t)mm * n + s.d.j[k]], px, py, pz);
+    }
+    __syncthreads();
+
+    // stage E: per-atom sums
+    for (int t = tid; t < na; t += pc::NT) {
+        const int64_t i = A0 + t;
+        T U = T(0), Fx = T(0), Fy = T(0), Fz = T(0);
+        T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+        for (int b = s.d.off[t]; b < s.d.off[t + 1]; ++b) {
+            const T px = s.Px[b], py = s.Py[b], pz = s.Pz[b];
+            U += s.fAu[b]; Fx += px; Fy += py; Fz += pz;
+            if (virial) {
+                const T rr = T(1) / s.rinv[b];
+                const T rx = s.d.ex[b] * rr, ry = s.d.ey[b] * rr, rz = s.d.ez[b] * rr;
+                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+            }
+        }
+        MASK[i] = s.d.mask[t];
+        if (pe) pe[i] = (double)U;
+        if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+        if (virial) {
+#pragma unroll
+            for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+        }
+    }
+}
+
 template <class T, class Rec>
 int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
            const double box[3], const md_tersoff_params* hp, double* pe, double* f, double* virial,
@@ -157,9 +443,35 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.w = (T)(3.14159265358979323846 / (hp->S - hp->R));
     p.minus_half_over_n = (T)(-0.5 / hp->n);
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
-    k_tersoff_pair<T, Rec><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(
-        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
-        pe, f, virial, nl->d_status);
+    const unsigned gb = (unsigned)((n + 127) / 128);
+#define MD_TERSOFF_LAUNCH(MRV)                                                                          \
+    k_tersoff_pair<T, Rec, MRV><<<gb, 128, 0, s>>>(n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,  \
+                                                   nl->REV, p, (Rec*)nl->Q, nl->MASK, pe, f, virial,    \
+                                                   nl->d_status)
+    static int mr = -1;
+    if (mr < 0) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 0; }
+    if (mr == 0) {
+        constexpr int TA = 64, PC = 8 * TA;
+        using Sm = TersoffSmem<T, TA, PC>;
+        auto kern = k_tersoff_pairs_cta<T, Rec, TA, PC>;
+        static bool attr_set = false;
+        if (!attr_set) {
+            MD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Sm)));
+            attr_set = true;
+        }
+        kern<<<(unsigned)((n + TA - 1) / TA), pc::NT, sizeof(Sm), s>>>(
+            n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
+            pe, f, virial, nl->d_status);
+        MD_CUDA_TRY(cudaGetLastError());
+        return MD_OK;
+    }
+    switch (mr) {
+        case 4: MD_TERSOFF_LAUNCH(4); break;
+        case 5: MD_TERSOFF_LAUNCH(5); break;
+        case 8: MD_TERSOFF_LAUNCH(8); break;
+        default: MD_TERSOFF_LAUNCH(6); break;
+    }
+#undef MD_TERSOFF_LAUNCH
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
 }
