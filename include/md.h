@@ -126,6 +126,11 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
  * the roofline.  Synchronous. */
 int md_probe_fp64_peak(int iters, double* tflops, void* stream);
 
+/* Diagnostic: out[k] = fn(in[k]) with the FP64 device functions the pair kernels use (fastmath.cuh):
+ * fn 0 exp, 1 log (in > 0, normal), 2 reciprocal, 3 reciprocal square root, 4 sin and 5 cos on [0, pi].
+ * DEVICE buffers of n doubles.  Lets a test bound their error against a long-double reference. */
+int md_math_probe(int fn, int64_t n, const double* in, double* out, void* stream);
+
 /* Per-kernel-kind device timing (CUDA events on the launching stream) and launch counts.
  * md_profile_enable(nl, 1) starts recording an event pair around every kernel group launched
  * through `nl`; md_profile_read synchronises the device, adds up the elapsed times and resets.

@@ -39,7 +39,7 @@ class md_sw_params(C.Structure):
 EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neighbors_status",
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
-           "md_profile_enable", "md_profile_read")
+           "md_profile_enable", "md_profile_read", "md_math_probe")
 
 _lib = None
 
@@ -212,6 +212,15 @@ def md_probe_fp64_peak(iters=20000, stream=None) -> float:
     t = C.c_double(0.0)
     _check(load().md_probe_fp64_peak(C.c_int(iters), C.byref(t), _stream(stream)), "md_probe_fp64_peak")
     return t.value
+
+
+MATH_FN = {"exp": 0, "log": 1, "rcp": 2, "rsqrt": 3, "sin": 4, "cos": 5}
+
+
+def md_math_probe(fn, n, inp, out, stream=None):
+    """out[k] = fn(inp[k]) with the pair kernels' FP64 device functions (DEVICE buffers)."""
+    _check(load().md_math_probe(C.c_int(MATH_FN[fn] if isinstance(fn, str) else fn), C.c_int64(n), _ptr(inp),
+                                _ptr(out), _stream(stream)), "md_math_probe")
 
 
 KINDS = ("build", "pair", "gather", "integrate")

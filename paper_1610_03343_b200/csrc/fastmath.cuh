@@ -1,105 +1,131 @@
 // fastmath.cuh -- branch-free FP64 elementary functions for the pair kernels.
 //
-// The pair kernels are bound by the FP64 pipe and by the latency of dependent DFMA chains.  The CUDA
-// library's exp/log carry range checks and slow-path branches that split basic blocks and stop ptxas
-// from interleaving the independent chains of an atom's neighbours.  These versions are straight-line
-// code valid on the ranges the potentials produce (stated per function); accuracy ~1-2 ulp, checked in
-// tests/test_gpu_math.py against mpmath.  The float overloads forward to the CUDA float functions.
+// The pair kernels are bound by the FP64 pipe (64 lanes per SM: a warp-wide FP64 instruction holds the
+// pipe of its SM sub-partition for two cycles), so what counts is the number of FP64 instructions and
+// that the code stays one straight basic block which ptxas can interleave across an atom's neighbours.
+// The CUDA library's exp/log spend 25-40 FP64 instructions each and carry range checks and slow-path
+// branches.  These versions use small tables (staged in shared memory, 1.5 KB) to shorten the
+// polynomials: exp 10 FP64 instructions, log 11.  Accuracy: |relative error| < 4e-16 (exp), absolute
+// error < 4e-16 * max(1, |log a|) (log) -- checked on the GPU against long-double references through
+// md_math_probe (tests/test_gpu_math.py).  The force tolerance is 1e-10, the energy tolerance 1e-12.
+// The float overloads forward to the CUDA float functions (FP32 mode is not FP64-pipe bound).
 #pragma once
 #include <cuda_runtime.h>
 
 namespace fm {
 
-// 1/a: MUFU.RCP64H seed + two Newton steps.  a normal, nonzero.
+constexpr int EXP_N = 64;                        // T[j] = 2^(j/64)
+constexpr int LOG_N = 64;                        // {c_j, -log c_j}, c_j ~ 1/(1 + (j + 1/2)/64)
+constexpr int TAB_DOUBLES = EXP_N + 2 * LOG_N;   // layout of md_neighbors::math_tab
+
+struct Tab {                                     // pointers into the shared-memory copy
+    const double* e;
+    const double2* l;
+};
+
+// Copies the tables from global to shared memory; the caller synchronises the block afterwards.
+__device__ __forceinline__ Tab stage_tables(double* smem /*[TAB_DOUBLES], 16-byte aligned*/,
+                                            const double* __restrict__ gtab) {
+    for (int k = threadIdx.x; k < TAB_DOUBLES; k += blockDim.x) smem[k] = gtab[k];
+    Tab t;
+    t.e = smem;
+    t.l = reinterpret_cast<const double2*>(smem + EXP_N);
+    return t;
+}
+
+// 1/a: MUFU.RCP64H seed, then one cubic step y (1 + e + e^2), e = 1 - a y.  a normal, nonzero.
 __device__ __forceinline__ double rcp(double a) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-    double e = __fma_rn(-a, y, 1.0);
-    y = __fma_rn(y, e, y);
-    e = __fma_rn(-a, y, 1.0);
-    return __fma_rn(y, e, y);
+    const double e = __fma_rn(-a, y, 1.0);
+    const double e2 = __fma_rn(e, e, e);
+    return __fma_rn(y, e2, y);
 }
 __device__ __forceinline__ float rcp(float a) { return __frcp_rn(a); }
 
-// 1/sqrt(a): MUFU.RSQ64H seed + two Newton steps.  a normal, positive.
+// 1/sqrt(a): MUFU.RSQ64H seed, then one cubic step y (1 + e/2 + 3 e^2/8), e = 1 - a y^2.
 __device__ __forceinline__ double rsqrt(double a) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-    double h = 0.5 * y;
-    double e = __fma_rn(-a * y, y, 1.0);
-    y = __fma_rn(h, e, y);
-    h = 0.5 * y;
-    e = __fma_rn(-a * y, y, 1.0);
-    return __fma_rn(h, e, y);
+    const double ay = a * y;
+    const double e = __fma_rn(-ay, y, 1.0);
+    const double t = __fma_rn(e, 0.375, 0.5) * e;
+    return __fma_rn(y, t, y);
 }
 __device__ __forceinline__ float rsqrt(float a) { return ::rsqrtf(a); }
 
-// exp(x) for x clamped to [-700, 700]: k = round(x/ln2), r = x - k ln2 (two-part), degree-13 Taylor
-// (|r| <= 0.3466: truncation 4e-18), scaled by adding k to the exponent field.
-__device__ __forceinline__ double exp(double x) {
-    x = fmin(fmax(x, -700.0), 700.0);
-    const double kd = __fma_rn(x, 1.4426950408889634, 6755399441055744.0);       // 1.5 * 2^52 trick
+// exp(x): k = round(64 x / ln 2), r = x - k ln2/64 (two parts, |r| <= 0.00542), degree-5 Taylor
+// (truncation 3.5e-17), times 2^(j/64) from the table with k >> 6 added to its exponent field.
+// Saturates instead of overflowing: the exponent shift is clamped to +-1020.
+__device__ __forceinline__ double exp(double x, const Tab& tb) {
+    const double kd = __fma_rn(x, 92.33248261689366, 6755399441055744.0);     // 1.5 * 2^52
     const int k = __double2loint(kd);
     const double kf = kd - 6755399441055744.0;
-    double r = __fma_rn(-kf, 0.6931471803691238, x);
-    r = __fma_rn(-kf, 1.9082149292705877e-10, r);
-    double p = 1.6059043836821613e-10;
-    p = __fma_rn(p, r, 2.08767569878681e-09);
-    p = __fma_rn(p, r, 2.505210838544172e-08);
-    p = __fma_rn(p, r, 2.755731922398589e-07);
-    p = __fma_rn(p, r, 2.7557319223985893e-06);
-    p = __fma_rn(p, r, 2.48015873015873e-05);
-    p = __fma_rn(p, r, 0.0001984126984126984);
-    p = __fma_rn(p, r, 0.001388888888888889);
-    p = __fma_rn(p, r, 0.008333333333333333);
-    p = __fma_rn(p, r, 0.041666666666666664);
+    double r = __fma_rn(kf, -0.01083042469326756, x);
+    r = __fma_rn(kf, -2.9815858269852933e-12, r);
+    double p = __fma_rn(r, 0.008333333333333333, 0.041666666666666664);
     p = __fma_rn(p, r, 0.16666666666666666);
     p = __fma_rn(p, r, 0.5);
     p = __fma_rn(p, r, 1.0);
     p = __fma_rn(p, r, 1.0);
-    // p in [0.70, 1.42]; 2^k with |k| <= 1010 split in two exact power-of-two multiplies
-    const int k1 = k >> 1, k2 = k - k1;
-    const double s1 = __hiloint2double((k1 + 1023) << 20, 0);
-    const double s2 = __hiloint2double((k2 + 1023) << 20, 0);
-    return p * s1 * s2;
+    const double t = tb.e[k & (EXP_N - 1)];
+    const int sh = max(-1020, min(1020, k >> 6));
+    const double s = __hiloint2double(__double2hiint(t) + (sh << 20), __double2loint(t));
+    return s * p;
 }
-__device__ __forceinline__ float exp(float x) { return ::expf(x); }
+__device__ __forceinline__ float exp(float x, const Tab&) { return ::expf(x); }
 
-// log(a) for a positive and normal: a = 2^e m, m in [sqrt(1/2), sqrt(2)); f = (m-1)/(m+1);
-// log m = 2 atanh f = 2f (1 + f^2/3 + ... + f^22/23), |f| <= 0.1716 (truncation 2e-19 relative).
-__device__ __forceinline__ double log(double a) {
-    int hi = __double2hiint(a);
-    const int lo = __double2loint(a);
-    int e = (hi >> 20) - 1023;
-    hi = (hi & 0x000fffff) | 0x3ff00000;                  // m in [1, 2)
-    double m = __hiloint2double(hi, lo);
-    if (m > 1.4142135623730951) { m *= 0.5; e += 1; }     // select, not a branch
-    const double f = (m - 1.0) * rcp(m + 1.0);
-    const double f2 = f * f;
-    double p = 0.08695652173913043;
-    p = __fma_rn(p, f2, 0.09523809523809523);
-    p = __fma_rn(p, f2, 0.10526315789473684);
-    p = __fma_rn(p, f2, 0.11764705882352941);
-    p = __fma_rn(p, f2, 0.13333333333333333);
-    p = __fma_rn(p, f2, 0.15384615384615385);
-    p = __fma_rn(p, f2, 0.18181818181818182);
-    p = __fma_rn(p, f2, 0.2222222222222222);
-    p = __fma_rn(p, f2, 0.2857142857142857);
-    p = __fma_rn(p, f2, 0.4);
-    p = __fma_rn(p, f2, 0.6666666666666666);
-    // log m = 2f + f * f2 * p
-    const double ed = (double)e;
-    const double t = __fma_rn(f * f2, p, ed * 1.9082149292705877e-10);
-    return __fma_rn(ed, 0.6931471803691238, __fma_rn(2.0, f, t));
+// log(a), a positive and normal: a = 2^e m, m in [1,2), j = top 6 mantissa bits,
+// r = m c_j - 1 (one FMA, |r| <= 1/128), log a = e ln2 - log c_j + log1p(r), degree-7 series.
+__device__ __forceinline__ double log(double a, const Tab& tb) {
+    const int hi = __double2hiint(a), lo = __double2loint(a);
+    const int e = (hi >> 20) - 1023;
+    const int j = (hi >> 14) & (LOG_N - 1);
+    const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
+    const double2 cl = tb.l[j];
+    const double r = __fma_rn(m, cl.x, -1.0);
+    double p = __fma_rn(r, 0.14285714285714285, -0.16666666666666666);
+    p = __fma_rn(p, r, 0.2);
+    p = __fma_rn(p, r, -0.25);
+    p = __fma_rn(p, r, 0.3333333333333333);
+    p = __fma_rn(p, r, -0.5);
+    // (double)e without I2F: 2^52 + 2^31 + e as a bit pattern, minus the bias
+    const double ed = __hiloint2double(0x43300000, e ^ 0x80000000) - 4503601774854144.0;
+    const double s = __fma_rn(ed, 0.6931471805599453, cl.y);
+    return s + __fma_rn(p, r * r, r);
 }
-__device__ __forceinline__ float log(float a) { return ::logf(a); }
+__device__ __forceinline__ float log(float a, const Tab&) { return ::logf(a); }
 
-// log(1 + t) for t >= 0 (and 1 + t normal): log(u) + (t - (u - 1))/u with u = fl(1 + t).
-__device__ __forceinline__ double log1p(double t) {
-    const double u = 1.0 + t;
-    const double c = (t - (u - 1.0)) * rcp(u);
-    return log(u) + c;
+// sin and cos of a in [0, pi] (the cut-off window's argument): q = round(2a/pi) in {0,1,2},
+// y = a - q pi/2 (two parts, |y| <= pi/4), Taylor series to y^15 / y^16.
+__device__ __forceinline__ void sincos_0_pi(double a, double* sn, double* cs) {
+    const double qd = __fma_rn(a, 0.6366197723675814, 6755399441055744.0);
+    const int q = __double2loint(qd);
+    const double qf = qd - 6755399441055744.0;
+    double y = __fma_rn(qf, -1.5707963109016418, a);
+    y = __fma_rn(qf, -1.5893254773528196e-08, y);
+    const double y2 = y * y;
+    double s = -7.647163731819816e-13;               // -1/15!
+    s = __fma_rn(s, y2, 1.6059043836821613e-10);     //  1/13!
+    s = __fma_rn(s, y2, -2.505210838544172e-08);     // -1/11!
+    s = __fma_rn(s, y2, 2.7557319223985893e-06);     //  1/9!
+    s = __fma_rn(s, y2, -0.0001984126984126984);     // -1/7!
+    s = __fma_rn(s, y2, 0.008333333333333333);       //  1/5!
+    s = __fma_rn(s, y2, -0.16666666666666666);       // -1/3!
+    s = __fma_rn(s * y2, y, y);
+    double c = 4.779477332387385e-14;                //  1/16!
+    c = __fma_rn(c, y2, -1.1470745597729725e-11);    // -1/14!
+    c = __fma_rn(c, y2, 2.08767569878681e-09);       //  1/12!
+    c = __fma_rn(c, y2, -2.755731922398589e-07);     // -1/10!
+    c = __fma_rn(c, y2, 2.48015873015873e-05);       //  1/8!
+    c = __fma_rn(c, y2, -0.001388888888888889);      // -1/6!
+    c = __fma_rn(c, y2, 0.041666666666666664);       //  1/4!
+    c = __fma_rn(c, y2, -0.5);
+    c = __fma_rn(c, y2, 1.0);
+    // q = 0: (s, c); q = 1: (c, -s); q = 2: (-s, -c)
+    *sn = q == 1 ? c : (q == 2 ? -s : s);
+    *cs = q == 1 ? -s : (q == 2 ? -c : c);
 }
-__device__ __forceinline__ float log1p(float t) { return ::log1pf(t); }
+__device__ __forceinline__ void sincos_0_pi(float a, float* sn, float* cs) { ::sincosf(a, sn, cs); }
 
 }  // namespace fm

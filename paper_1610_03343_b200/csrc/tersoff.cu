@@ -12,6 +12,7 @@
 #include "common.cuh"
 #include "real_math.cuh"
 #include "pair_cta.cuh"
+#include "fastmath.cuh"
 
 namespace {
 
@@ -150,29 +151,33 @@ tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const d
     }
 }
 
-// 1/a by MUFU.RCP64H + two Newton steps (4 DFMA): full double accuracy for normal a, no IEEE special cases.
-__device__ __forceinline__ double fast_rcp(double a) {
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
-    double e = __fma_rn(-a, y, 1.0);
-    y = __fma_rn(y, e, y);
-    e = __fma_rn(-a, y, 1.0);
-    return __fma_rn(y, e, y);
+// Minimum image of a difference that is known to lie within the list cut-off of 0 or of +-L (a listed
+// pair, coordinates in [0, L)): any threshold between works, so the test is an integer compare on the
+// high word (no FP64-pipe instruction) and the shift one DADD.
+__device__ __forceinline__ double min_image_listed(double d, double L, int hi_half) {
+    const int hi = __double2hiint(d);
+    const int sL = __double2hiint(L) | (hi & 0x80000000);            // copysign(L, d), high word
+    const double shift = (hi & 0x7fffffff) > hi_half ? __hiloint2double(sL, __double2loint(L)) : 0.0;
+    return d - shift;
 }
-__device__ __forceinline__ float fast_rcp(float a) { return __frcp_rn(a); }
 
 // Register path: list rows of up to MR entries, every per-neighbour quantity in registers (all array
-// indices are compile-time constants after unrolling; slots m >= nn are skipped by warp-uniform branches).
-// A listed neighbour outside the force range keeps f_C = f_C' = f_R = f_A = 0, so it drops out of every sum.
-template <class T, class Rec, int MR>
-__global__ void __launch_bounds__(128)
-k_tersoff_pair(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+// indices are compile-time constants after unrolling).  The arithmetic is one straight basic block over
+// all MR slots, so ptxas interleaves the slots' independent FP64 chains; a slot that is empty or outside
+// the force range carries f_C = f_C' = f_R = f_A = 0 and drops out of every sum.  The only branch is the
+// (rare) cut-off window R < r < S.
+template <class T, class Rec, int MR, int MINB>
+__global__ void __launch_bounds__(128, MINB)
+k_tersoff_atom(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                const double* __restrict__ z, double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, TersoffDev<T> p,
+               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                int* __restrict__ status) {
+    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    __syncthreads();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int nn = NN[i];
@@ -181,109 +186,112 @@ k_tersoff_pair(int64_t n, const double* __restrict__ x, const double* __restrict
         return;
     }
     const double xi = x[i], yi = y[i], zi = z[i];
-    const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
+    const int hhx = __double2hiint(0.5 * Lx), hhy = __double2hiint(0.5 * Ly), hhz = __double2hiint(0.5 * Lz);
 
-    int jd[MR];
+    int jd[MR], rv[MR];
     double dx[MR], dy[MR], dz[MR];
 #pragma unroll
-    for (int m = 0; m < MR; ++m) jd[m] = m < nn ? NL[(int64_t)m * n + i] : (int)i;
+    for (int m = 0; m < MR; ++m) {
+        jd[m] = m < nn ? NL[(int64_t)m * n + i] : (int)i;
+        rv[m] = m < nn ? (int)REV[(int64_t)m * n + i] : 0;
+    }
 #pragma unroll
     for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
 
-    T ex[MR], ey[MR], ez[MR], rinv[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
-    unsigned mask = 0u;
+    T ex[MR], ey[MR], ez[MR], rinv[MR], rr[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
+    unsigned mask = 0u, window = 0u;
 #pragma unroll
     for (int m = 0; m < MR; ++m) {
-        ex[m] = ey[m] = ez[m] = rinv[m] = fc[m] = fcp[m] = fR[m] = fA[m] = zeta[m] = T(0);
-        if (m < nn) {
-            const T tx = (T)md_min_image(dx[m] - xi, Lx, hx);
-            const T ty = (T)md_min_image(dy[m] - yi, Ly, hy);
-            const T tz = (T)md_min_image(dz[m] - zi, Lz, hz);
-            const T d2 = tx * tx + ty * ty + tz * tz;
-            const T ri = rm::rsqrt(d2);
-            const T rr = d2 * ri;
-            ex[m] = tx * ri; ey[m] = ty * ri; ez[m] = tz * ri; rinv[m] = ri;
-            if (d2 < p.S2) {
-                mask |= 1u << m;
-                T c = T(1), cp = T(0);
-                if (rr > p.R) {                              // f_C window R < r < S (reading A1)
-                    T sn, cs;
-                    rm::sincos((rr - p.R) * p.w, &sn, &cs);
-                    c = T(0.5) + T(0.5) * cs;
-                    cp = T(-0.5) * p.w * sn;
-                }
-                fc[m] = c; fcp[m] = cp;
-                fR[m] = p.A * rm::exp(-p.lambda * rr);
-                fA[m] = p.B * rm::exp(-p.mu * rr);
+        const T tx = (T)min_image_listed(dx[m] - xi, Lx, hhx);
+        const T ty = (T)min_image_listed(dy[m] - yi, Ly, hhy);
+        const T tz = (T)min_image_listed(dz[m] - zi, Lz, hhz);
+        const T d2 = tx * tx + ty * ty + tz * tz;
+        const bool in = m < nn && d2 < p.S2;
+        const T d2s = in ? d2 : T(1);                        // keeps the empty slot's arithmetic finite
+        const T ri = fm::rsqrt(d2s);
+        rr[m] = d2s * ri;
+        ex[m] = tx * ri; ey[m] = ty * ri; ez[m] = tz * ri; rinv[m] = ri;
+        mask |= in ? 1u << m : 0u;
+        window |= (in && rr[m] > p.R) ? 1u << m : 0u;
+        fc[m] = in ? T(1) : T(0);
+        fcp[m] = T(0);
+        const T eR = fm::exp(-p.lambda * rr[m], tb), eA = fm::exp(-p.mu * rr[m], tb);
+        fR[m] = in ? p.A * eR : T(0);
+        fA[m] = in ? p.B * eA : T(0);
+        zeta[m] = T(0);
+    }
+    if (window) {                                            // f_C window R < r < S (reading A1)
+#pragma unroll
+        for (int m = 0; m < MR; ++m)
+            if (window >> m & 1u) {
+                T sn, cs;
+                fm::sincos_0_pi((rr[m] - p.R) * p.w, &sn, &cs);
+                fc[m] = T(0.5) + T(0.5) * cs;
+                fcp[m] = T(-0.5) * p.w * sn;
             }
-        }
     }
 
-    // zeta (Eq. 4), unordered neighbour pairs visited once (g_ijk = g_ikj for one element)
+    // zeta (Eq. 4), unordered neighbour pairs visited once (g_ijk = g_ikj for one element);
+    // g = 1 + (c/d)^2 x^2/(d^2 + x^2), x = h - cos (Eq. 5 without its cancellation)
 #pragma unroll
     for (int a = 0; a < MR; ++a)
 #pragma unroll
-        for (int b = a + 1; b < MR; ++b)
-            if (b < nn) {
-                const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-                const T xx = p.h - cs;
-                const T x2 = xx * xx;
-                const T g = T(1) + p.c2_over_d2 * x2 * fast_rcp(p.d2 + x2);
-                zeta[a] += fc[b] * g;
-                zeta[b] += fc[a] * g;
-            }
+        for (int b = a + 1; b < MR; ++b) {
+            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+            const T xx = p.h - cs;
+            const T x2 = xx * xx;
+            const T g = T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2);
+            zeta[a] += fc[b] * g;
+            zeta[b] += fc[a] * g;
+        }
 
+    // b_ij, b'_ij (Eq. 3); zeta = 0: b = 1, b' = 0 (reading A8)
     T U = T(0);
     T Px[MR], Py[MR], Pz[MR], hh[MR];
 #pragma unroll
     for (int a = 0; a < MR; ++a) {
-        Px[a] = Py[a] = Pz[a] = hh[a] = T(0);
-        if (a < nn && (mask >> a & 1u)) {
-            T b = T(1), bp = T(0);
-            const T zt = zeta[a];
-            if (zt > T(0)) {                                 // zeta = 0: b = 1, b' = 0 (reading A8)
-                const T t = rm::exp(p.n * rm::log(p.beta * zt));
-                b = rm::exp(p.minus_half_over_n * rm::log1p(t));
-                bp = T(-0.5) * b * t * fast_rcp(zt * (T(1) + t));
-            }
-            const T bfA = b * fA[a];
-            U += T(0.5) * fc[a] * (fR[a] - bfA);
-            const T D = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
-            hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
-            Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
-        }
+        const bool pos = zeta[a] > T(0);
+        const T zt = pos ? zeta[a] : T(1);
+        const T t = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);        // (beta zeta)^n
+        const T u = T(1) + t;
+        const T bb = fm::exp(p.minus_half_over_n * fm::log(u, tb), tb); // (1 + t)^(-1/2n)
+        const T b = pos ? bb : T(1);
+        const T bp = pos ? T(-0.5) * bb * t * fm::rcp(zt * u) : T(0);
+        const T bfA = b * fA[a];
+        U += T(0.5) * fc[a] * (fR[a] - bfA);
+        const T D = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
+        hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
+        Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
     }
 
+    // P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g'_ab (e_b - cos e_a)/r_a + h_b fc'_a g_ab e_a ]
 #pragma unroll
     for (int a = 0; a < MR; ++a)
 #pragma unroll
-        for (int b = a + 1; b < MR; ++b)
-            if (b < nn) {
-                const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-                const T xx = p.h - cs;
-                const T x2 = xx * xx;
-                const T q = fast_rcp(p.d2 + x2);
-                const T g = T(1) + p.c2_over_d2 * x2 * q;
-                const T gp = T(-2) * p.c2 * xx * q * q;      // dg/dcos
-                const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
-                const T ta = tab * rinv[a], tb = tab * rinv[b];
-                const T ua = hh[b] * fcp[a] * g - ta * cs;
-                const T ub = hh[a] * fcp[b] * g - tb * cs;
-                Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
-                Px[b] += tb * ex[a] + ub * ex[b]; Py[b] += tb * ey[a] + ub * ey[b]; Pz[b] += tb * ez[a] + ub * ez[b];
-            }
+        for (int b = a + 1; b < MR; ++b) {
+            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+            const T xx = p.h - cs;
+            const T x2 = xx * xx;
+            const T q = fm::rcp(p.d2 + x2);
+            const T g = T(1) + p.c2_over_d2 * x2 * q;
+            const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
+            const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
+            const T ta = tab * rinv[a], tb2 = tab * rinv[b];
+            const T ua = hh[b] * fcp[a] * g - ta * cs;
+            const T ub = hh[a] * fcp[b] * g - tb2 * cs;
+            Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
+            Px[b] += tb2 * ex[a] + ub * ex[b]; Py[b] += tb2 * ey[a] + ub * ey[b]; Pz[b] += tb2 * ez[a] + ub * ez[b];
+        }
 
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
 #pragma unroll
     for (int a = 0; a < MR; ++a)
-        if (a < nn && (mask >> a & 1u)) {
-            const int mm = REV[(int64_t)a * n + i];
-            rm::store_rec(&Q[(int64_t)mm * n + jd[a]], Px[a], Py[a], Pz[a]);
+        if (mask >> a & 1u) {
+            rm::store_rec(&Q[(int64_t)rv[a] * n + jd[a]], Px[a], Py[a], Pz[a]);
             Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
             if (virial) {
-                const T rr = T(1) / rinv[a];
-                const T rx = ex[a] * rr, ry = ey[a] * rr, rz = ez[a] * rr;
+                const T rx = ex[a] * rr[a], ry = ey[a] * rr[a], rz = ez[a] * rr[a];
                 W[0] += rx * Px[a]; W[1] += rx * Py[a]; W[2] += rx * Pz[a];
                 W[3] += ry * Px[a]; W[4] += ry * Py[a]; W[5] += ry * Pz[a];
                 W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
@@ -444,12 +452,14 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.minus_half_over_n = (T)(-0.5 / hp->n);
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const unsigned gb = (unsigned)((n + 127) / 128);
-#define MD_TERSOFF_LAUNCH(MRV)                                                                          \
-    k_tersoff_pair<T, Rec, MRV><<<gb, 128, 0, s>>>(n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,  \
-                                                   nl->REV, p, (Rec*)nl->Q, nl->MASK, pe, f, virial,    \
-                                                   nl->d_status)
+    const double* gtab = md_math_tables();
+    if (!gtab) return MD_ERR_ALLOC;
+#define MD_TERSOFF_LAUNCH(MRV, MINB)                                                                      \
+    k_tersoff_atom<T, Rec, MRV, MINB><<<gb, 128, 0, s>>>(n, x, y, z, box[0], box[1], box[2], nl->NN,    \
+                                                         nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,          \
+                                                         nl->MASK, pe, f, virial, nl->d_status)
     static int mr = -1;
-    if (mr < 0) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 0; }
+    if (mr < 0) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 4; }
     if (mr == 0) {
         constexpr int TA = 64, PC = 8 * TA;
         using Sm = TersoffSmem<T, TA, PC>;
@@ -466,10 +476,11 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         return MD_OK;
     }
     switch (mr) {
-        case 4: MD_TERSOFF_LAUNCH(4); break;
-        case 5: MD_TERSOFF_LAUNCH(5); break;
-        case 8: MD_TERSOFF_LAUNCH(8); break;
-        default: MD_TERSOFF_LAUNCH(6); break;
+        case 43: MD_TERSOFF_LAUNCH(4, 3); break;
+        case 45: MD_TERSOFF_LAUNCH(4, 5); break;
+        case 5: MD_TERSOFF_LAUNCH(5, 3); break;
+        case 6: MD_TERSOFF_LAUNCH(6, 2); break;
+        default: MD_TERSOFF_LAUNCH(4, 4); break;
     }
 #undef MD_TERSOFF_LAUNCH
     MD_CUDA_TRY(cudaGetLastError());
