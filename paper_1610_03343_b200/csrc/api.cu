@@ -10,7 +10,7 @@ bool valid_box(const double box[3]) { return box && box[0] > 0 && box[1] > 0 && 
 
 void free_all(md_neighbors* nl) {
     cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
-    cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted);
+    cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e);
     if (nl->ev_pool) for (cudaEvent_t e : *nl->ev_pool) cudaEventDestroy(e);
     delete nl->ev_pool; delete nl->ev_kind;
@@ -19,12 +19,12 @@ void free_all(md_neighbors* nl) {
 int force_dispatch(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                    const double* x, const double* y, const double* z, const double* vx, const double* vy,
                    const double* vz, const double box[3], double* pe, double* f, double* virial,
-                   double* heat, cudaStream_t s) {
+                   double* heat, const VVFuse* vv, cudaStream_t s) {
     if (potential == MD_TERSOFF)
         return md_launch_tersoff(nl, n, x, y, z, vx, vy, vz, box, (const md_tersoff_params*)params, precision,
-                                 pe, f, virial, heat, s);
+                                 pe, f, virial, heat, vv, s);
     return md_launch_sw(nl, n, x, y, z, vx, vy, vz, box, (const md_sw_params*)params, precision, pe, f,
-                        virial, heat, s);
+                        virial, heat, vv, s);
 }
 
 int check_force_args(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
@@ -112,6 +112,7 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->cell_of, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->rank_in_cell, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->sortedf, n * sizeof(float4)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->d_status, 2 * sizeof(int)) == cudaSuccess;
     if (!ok) { cudaGetLastError(); free_all(nl); delete nl; return MD_ERR_ALLOC; }
     cudaMemset(nl->d_status, 0, 2 * sizeof(int));
@@ -175,7 +176,7 @@ int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double*
     int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
     if (rc != MD_OK) return rc;
     if (!(p->S > p->R) || !(p->R > 0) || !(p->n > 0) || !(p->d != 0)) return MD_ERR_ARG;
-    return md_launch_tersoff(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat,
+    return md_launch_tersoff(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat, nullptr,
                              (cudaStream_t)stream);
 }
 
@@ -186,7 +187,7 @@ int md_sw_force(md_neighbors* nl, int64_t n, const double* x, const double* y, c
     int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
     if (rc != MD_OK) return rc;
     if (!(p->sigma > 0) || !(p->a > 0)) return MD_ERR_ARG;
-    return md_launch_sw(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat,
+    return md_launch_sw(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat, nullptr,
                         (cudaStream_t)stream);
 }
 
@@ -215,17 +216,24 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
     if (!f_valid) {
         if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
-                                 pe, f, nullptr, nullptr, s)) != MD_OK) return rc;
+                                 pe, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
     }
+    if (nsteps == 0) return MD_OK;
+    // Step s = kick+drift, [rebuild], force, kick.  The kick that ends step s and the kick+drift that
+    // starts step s+1 are fused into the gather kernel of step s (gather.cu, k_gather_vv): per step the
+    // loop launches the pair kernel and one fused kernel, plus the list build on rebuild steps.
+    VVFuse vv;
+    vv.hk = 0.5 * dt_fs * MD_KAPPA / mass_amu; vv.dt = dt_fs;
+    vv.x = x; vv.y = y; vv.z = z; vv.vx = vx; vv.vy = vy; vv.vz = vz;
+    if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
     for (int step = first_step; step < first_step + nsteps; ++step) {
-        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
         if (step % rebuild_every == 0)
             if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if (nl->n != n) return MD_ERR_NO_LIST;
         const bool last = step == first_step + nsteps - 1;
+        vv.mode = last ? 1 : 2;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
-                                 last ? pe : nullptr, f, nullptr, nullptr, s)) != MD_OK) return rc;
-        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+                                 last ? pe : nullptr, f, nullptr, nullptr, &vv, s)) != MD_OK) return rc;
     }
     return MD_OK;
 }

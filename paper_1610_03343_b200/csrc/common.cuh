@@ -43,6 +43,7 @@ struct md_neighbors {
     int32_t* cell_of;       // [n]
     int32_t* rank_in_cell;  // [n]
     double4* sorted;        // [n] {x,y,z, index bits} in cell order
+    float4* sortedf;        // [n] the same in float (FP32 screen of the candidate search)
     int32_t* scan_blocks;   // block sums scratch
     // status
     int* d_status;          // [2]: status bits, max row length seen
@@ -65,6 +66,22 @@ __device__ __forceinline__ double md_min_image(double d, double L, double halfL)
     return d;
 }
 
+// velocity-Verlet pieces shared by integrate.cu and the fused gather kernel
+constexpr double MD_KAPPA = 9.648533215665e-3;   // (A/fs^2) per (eV/A/amu)
+__device__ __forceinline__ double md_wrap(double c, double L) {
+    c -= L * floor(c / L);
+    return (c >= L || c < 0.0) ? 0.0 : c;        // reading A8
+}
+// What md_nve_run fuses into the gather kernel after the force is complete (nullptr = nothing):
+//   mode 1: v += hk F                                  (second half-kick of the step; F is stored)
+//   mode 2: v += hk F; v += hk F; x += dt v; wrap      (that kick and the next step's kick+drift; F is
+//           not stored: nothing reads it before the next force evaluation overwrites it)
+struct VVFuse {
+    int mode;
+    double hk, dt;
+    double *x, *y, *z, *vx, *vy, *vz;
+};
+
 // RAII scope: counts `nk` kernel launches of `kind` and, if profiling is on, brackets them with events.
 struct ProfScope {
     md_neighbors* nl; cudaStream_t s; cudaEvent_t e1; bool on;
@@ -79,14 +96,14 @@ int md_launch_reverse(md_neighbors* nl, cudaStream_t s);
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
-                      double* heat, cudaStream_t s);
+                      double* heat, const VVFuse* vv, cudaStream_t s);
 int md_launch_sw(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                  const double* vx, const double* vy, const double* vz, const double box[3],
                  const md_sw_params* p, int precision, double* pe, double* f, double* virial,
-                 double* heat, cudaStream_t s);
+                 double* heat, const VVFuse* vv, cudaStream_t s);
 int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                      const double* vx, const double* vy, const double* vz, const double box[3],
-                     int precision, double* f, double* virial, double* heat, cudaStream_t s);
+                     int precision, double* f, double* virial, double* heat, const VVFuse* vv, cudaStream_t s);
 int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s);
 const double* md_math_tables();   // device tables of fastmath.cuh for the current device (nullptr on failure)

@@ -61,14 +61,63 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
     if (heat) { heat[i] = (double)Jx; heat[n + i] = (double)Jy; heat[2 * n + i] = (double)Jz; }
 }
 
+// The same force sum with the velocity-Verlet half steps that follow it fused in (md_nve_run only, where
+// neither virial nor heat current is asked for): F_i is complete in registers, so the second half-kick of
+// this step and, unless it is the last step, the next step's kick + drift + wrap are applied before
+// anything is stored.  The arithmetic is operation for operation that of k_gather followed by k_kick and
+// k_kick_drift (integrate.cu), so the trajectory is bit-identical to the unfused composition.
+template <class T, class Rec, int MODE>
+__global__ void __launch_bounds__(256)
+k_gather_vv(int64_t n, const Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+            double* __restrict__ f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
+            double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
+            double hk, double dt, double Lx, double Ly, double Lz) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned long long mask = MASK[i];
+    const double ox = f[i], oy = f[n + i], oz = f[2 * n + i];           // own halves sum_j P_ij
+    double ux = vx[i], uy = vy[i], uz = vz[i];
+    double px = 0, py = 0, pz = 0;
+    if (MODE == 2) { px = x[i]; py = y[i]; pz = z[i]; }
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    while (mask) {
+        const int m = __ffsll((long long)mask) - 1;
+        mask &= mask - 1;
+        T qx, qy, qz;
+        rm::load_rec(&Q[(int64_t)m * n + i], &qx, &qy, &qz);
+        Fx += qx; Fy += qy; Fz += qz;
+    }
+    const double fx = ox - (double)Fx, fy = oy - (double)Fy, fz = oz - (double)Fz;
+    ux = __fma_rn(hk, fx, ux); uy = __fma_rn(hk, fy, uy); uz = __fma_rn(hk, fz, uz);     // kick of this step
+    if (MODE == 1) { f[i] = fx; f[n + i] = fy; f[2 * n + i] = fz; }
+    if (MODE == 2) {
+        ux = __fma_rn(hk, fx, ux); uy = __fma_rn(hk, fy, uy); uz = __fma_rn(hk, fz, uz); // kick of the next
+        x[i] = md_wrap(__fma_rn(dt, ux, px), Lx);
+        y[i] = md_wrap(__fma_rn(dt, uy, py), Ly);
+        z[i] = md_wrap(__fma_rn(dt, uz, pz), Lz);
+    }
+    vx[i] = ux; vy[i] = uy; vz[i] = uz;
+}
+
 }  // namespace
 
 int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                      const double* vx, const double* vy, const double* vz, const double box[3],
-                     int precision, double* f, double* virial, double* heat, cudaStream_t s) {
+                     int precision, double* f, double* virial, double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0 || (!f && !virial && !heat)) return MD_OK;
     const unsigned gb = (unsigned)((n + 255) / 256);
     ProfScope prof(nl, MD_KIND_GATHER, 1, s);
+    if (vv) {
+        if (!f || virial || heat) return MD_ERR_ARG;
+#define MD_GATHER_VV(TT, RR, MODE)                                                                        \
+    k_gather_vv<TT, RR, MODE><<<gb, 256, 0, s>>>(n, (const RR*)nl->Q, nl->MASK, f, vv->x, vv->y, vv->z,   \
+                                                 vv->vx, vv->vy, vv->vz, vv->hk, vv->dt, box[0], box[1], box[2])
+        if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }
+        else { if (vv->mode == 2) MD_GATHER_VV(double, PairRec64, 2); else MD_GATHER_VV(double, PairRec64, 1); }
+#undef MD_GATHER_VV
+        MD_CUDA_TRY(cudaGetLastError());
+        return MD_OK;
+    }
     if (precision == MD_FP32)
         k_gather<float, float4><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
                                                    (const float4*)nl->Q, nl->MASK, f, virial, heat);

@@ -2,12 +2,6 @@
 #include "common.cuh"
 
 namespace {
-constexpr double KAPPA = 9.648533215665e-3;   // (A/fs^2) per (eV/A/amu)
-
-__device__ __forceinline__ double wrap(double c, double L) {
-    c -= L * floor(c / L);
-    return (c >= L || c < 0.0) ? 0.0 : c;      // reading A8
-}
 
 __global__ void k_kick_drift(int64_t n, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
                              double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
@@ -16,9 +10,9 @@ __global__ void k_kick_drift(int64_t n, double* __restrict__ x, double* __restri
     if (i >= n) return;
     const double ux = __fma_rn(hk, f[i], vx[i]) , uy = __fma_rn(hk, f[n + i], vy[i]), uz = __fma_rn(hk, f[2 * n + i], vz[i]);
     vx[i] = ux; vy[i] = uy; vz[i] = uz;
-    x[i] = wrap(__fma_rn(dt, ux, x[i]), Lx);
-    y[i] = wrap(__fma_rn(dt, uy, y[i]), Ly);
-    z[i] = wrap(__fma_rn(dt, uz, z[i]), Lz);
+    x[i] = md_wrap(__fma_rn(dt, ux, x[i]), Lx);
+    y[i] = md_wrap(__fma_rn(dt, uy, y[i]), Ly);
+    z[i] = md_wrap(__fma_rn(dt, uz, z[i]), Lz);
 }
 
 __global__ void k_kick(int64_t n, double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
@@ -34,7 +28,7 @@ __global__ void k_kick(int64_t n, double* __restrict__ vx, double* __restrict__ 
 int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s) {
     if (n == 0) return MD_OK;
-    const double hk = 0.5 * dt * KAPPA / mass;
+    const double hk = 0.5 * dt * MD_KAPPA / mass;
     const unsigned gb = (unsigned)((n + 255) / 256);
     ProfScope prof(nl, MD_KIND_INTEGRATE, 1, s);
     if (phase == 0) k_kick_drift<<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, f, hk, dt, box[0], box[1], box[2]);

@@ -2,9 +2,14 @@
 //
 //   k_bin      cell id per atom + histogram (integer atomics; the force path has none)
 //   k_scan_*   exclusive prefix sum of the histogram with warp-shuffle scans (counting sort)
-//   k_scatter  atoms -> cell order as 32-byte {x,y,z,index} records
-//   k_search   one thread per atom (cell order): 27-cell search, strict d2 < r_list^2,
-//              row sorted by index, neighbour-major store NL[m*n+i]
+//   k_scatter  atoms -> cell order as 32-byte {x,y,z,index} records, plus a 16-byte float copy
+//   k_search   one thread per atom (cell order): 27-cell search.  Candidates are screened in FP32 on
+//              the float copy (the FP64 pipe would otherwise bound the build: ~58 candidates x ~15
+//              FP64 instructions per atom, more than the Tersoff force itself); the few that pass are
+//              decided by the canonical FP64 predicate, strict d2 < r_list^2.  The z-neighbour cells
+//              of a column are contiguous in cell order, so an interior atom scans 9 ranges, not 27.
+//              Rows are kept sorted by index in a shared-memory scratch [K][128] (no local memory) and
+//              stored neighbour-major, NL[m*n+i]
 //   k_reverse  REV[m*n+i] = position of i in row NL[m*n+i]
 #include "common.cuh"
 
@@ -115,36 +120,61 @@ __global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t*
 __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                           const double* __restrict__ z, const int32_t* __restrict__ cell_of,
                           const int32_t* __restrict__ rank, const int32_t* __restrict__ cell_start,
-                          double4* __restrict__ sorted) {
+                          double4* __restrict__ sorted, float4* __restrict__ sortedf) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int pos = cell_start[cell_of[i]] + rank[i];
-    sorted[pos] = make_double4(x[i], y[i], z[i], __longlong_as_double((long long)i));
+    const double xi = x[i], yi = y[i], zi = z[i];
+    sorted[pos] = make_double4(xi, yi, zi, __longlong_as_double((long long)i));
+    sortedf[pos] = make_float4((float)xi, (float)yi, (float)zi, __int_as_float((int)i));
 }
 
-__global__ void __launch_bounds__(128)
-k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const int32_t* __restrict__ cell_of,
-         const int32_t* __restrict__ cell_start, int K, int32_t* __restrict__ NN,
+constexpr int SEARCH_BT = 128;
+
+__global__ void __launch_bounds__(SEARCH_BT)
+k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __restrict__ sortedf,
+         const int32_t* __restrict__ cell_start, int K, float rc2_screen, int32_t* __restrict__ NN,
          int32_t* __restrict__ NL, int* __restrict__ status) {
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    extern __shared__ int s_nb[];                            // [K][SEARCH_BT]: this thread's row, sorted
+    const int tid = threadIdx.x;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + tid;
     if (t >= n) return;
     const double4 a = sorted[t];
     const int i = (int)__double_as_longlong(a.w);
-    const int c = cell_of[i];
-    const int cz = c % g.nc[2];
-    const int cy = (c / g.nc[2]) % g.nc[1];
-    const int cx = c / (g.nc[2] * g.nc[1]);
-    int nb[MD_MAX_NEIGHBORS];
+    const float xf = (float)a.x, yf = (float)a.y, zf = (float)a.z;
+    const int cx = cell_coord(a.x, g.inv_cell[0], g.nc[0]);  // as in k_bin, bit for bit
+    const int cy = cell_coord(a.y, g.inv_cell[1], g.nc[1]);
+    const int cz = cell_coord(a.z, g.inv_cell[2], g.nc[2]);
+    const float Lxf = (float)g.L[0], Lyf = (float)g.L[1], Lzf = (float)g.L[2];
+    const bool interior_z = cz > 0 && cz < g.nc[2] - 1;
     int cnt = 0;
     for (int ox = -1; ox <= 1; ++ox) {
-        int ax = cx + ox; ax = ax < 0 ? ax + g.nc[0] : (ax >= g.nc[0] ? ax - g.nc[0] : ax);
+        int ax = cx + ox;
+        float xs = xf;                                       // reference shifted instead of the candidate
+        if (ax < 0) { ax += g.nc[0]; xs += Lxf; } else if (ax >= g.nc[0]) { ax -= g.nc[0]; xs -= Lxf; }
         for (int oy = -1; oy <= 1; ++oy) {
-            int ay = cy + oy; ay = ay < 0 ? ay + g.nc[1] : (ay >= g.nc[1] ? ay - g.nc[1] : ay);
-            for (int oz = -1; oz <= 1; ++oz) {
-                int az = cz + oz; az = az < 0 ? az + g.nc[2] : (az >= g.nc[2] ? az - g.nc[2] : az);
-                const int cc = (ax * g.nc[1] + ay) * g.nc[2] + az;
-                const int beg = cell_start[cc], end = cell_start[cc + 1];
+            int ay = cy + oy;
+            float ys = yf;
+            if (ay < 0) { ay += g.nc[1]; ys += Lyf; } else if (ay >= g.nc[1]) { ay -= g.nc[1]; ys -= Lyf; }
+            const int base = (ax * g.nc[1] + ay) * g.nc[2];
+            // one contiguous range for an interior atom, else the three z cells one by one
+            const int nseg = interior_z ? 1 : 3;
+            for (int sg = 0; sg < nseg; ++sg) {
+                int beg, end;
+                float zs = zf;
+                if (interior_z) {
+                    beg = cell_start[base + cz - 1];
+                    end = cell_start[base + cz + 2];
+                } else {
+                    int az = cz + sg - 1;
+                    if (az < 0) { az += g.nc[2]; zs += Lzf; } else if (az >= g.nc[2]) { az -= g.nc[2]; zs -= Lzf; }
+                    beg = cell_start[base + az];
+                    end = cell_start[base + az + 1];
+                }
                 for (int q = beg; q < end; ++q) {
+                    const float4 bf = sortedf[q];
+                    const float fx = bf.x - xs, fy = bf.y - ys, fz = bf.z - zs;
+                    if (fmaf(fz, fz, fmaf(fy, fy, fx * fx)) >= rc2_screen) continue;    // FP32 screen
                     const double4 b = sorted[q];
                     const int j = (int)__double_as_longlong(b.w);
                     // canonical predicate (reading A7): explicit roundings, no contraction
@@ -155,8 +185,11 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const int32_t* _
                     if (d2 < g.rc2 && j != i) {
                         if (cnt < K) {
                             int p = cnt;                      // insertion keeps the row sorted by j
-                            while (p > 0 && nb[p - 1] > j) { nb[p] = nb[p - 1]; --p; }
-                            nb[p] = j;
+                            while (p > 0 && s_nb[(p - 1) * SEARCH_BT + tid] > j) {
+                                s_nb[p * SEARCH_BT + tid] = s_nb[(p - 1) * SEARCH_BT + tid];
+                                --p;
+                            }
+                            s_nb[p * SEARCH_BT + tid] = j;
                         }
                         ++cnt;
                     }
@@ -167,7 +200,7 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const int32_t* _
     atomicMax(&status[1], cnt);
     if (cnt > K) { atomicOr(&status[0], MD_DEV_ROW_OVERFLOW); cnt = K; }
     NN[i] = cnt;
-    for (int m = 0; m < cnt; ++m) NL[(int64_t)m * n + i] = nb[m];
+    for (int m = 0; m < cnt; ++m) NL[(int64_t)m * n + i] = s_nb[m * SEARCH_BT + tid];
 }
 
 __global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
@@ -232,9 +265,15 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     k_scan_local<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks);
     k_scan_tiles<<<1, 1024, 0, s>>>(nl->scan_blocks, ntiles);
     k_scan_add<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks, (int32_t)n);
-    k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted);
-    k_search<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, g, nl->sorted, nl->cell_of, nl->cell_count, nl->K,
-                                                       nl->NN, nl->NL, nl->d_status);
+    k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted,
+                                 nl->sortedf);
+    // FP32 screen: float coordinates carry an absolute error <= 2^-24 max(L) each, so |d2_f32 - d2| is
+    // below 4 (r_list + e) e + rounding with e = 3 * 2^-23 max(L); the margin below is 4x that bound.
+    const double Lmax = fmax(box[0], fmax(box[1], box[2]));
+    const double e = 3.0 * Lmax * 1.1920929e-7;
+    const float rc2_screen = (float)(g.rc2 + 16.0 * (r_list + e) * e + 1e-6 * g.rc2);
+    k_search<<<(unsigned)((n + SEARCH_BT - 1) / SEARCH_BT), SEARCH_BT, sizeof(int) * SEARCH_BT * nl->K, s>>>(
+        n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K, rc2_screen, nl->NN, nl->NL, nl->d_status);
     }
     MD_CUDA_TRY(cudaGetLastError());
     return md_launch_reverse(nl, s);

@@ -146,10 +146,10 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
 int md_launch_sw(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                  const double* vx, const double* vy, const double* vz, const double box[3],
                  const md_sw_params* p, int precision, double* pe, double* f, double* virial,
-                 double* heat, cudaStream_t s) {
+                 double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0) return MD_OK;
     int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, s)
                                   : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, s);
     if (rc != MD_OK) return rc;
-    return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, s);
+    return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, vv, s);
 }

@@ -7,6 +7,7 @@
 //     (Q[rev(i,m)*n + j]; exactly one writer per slot, no atomics),
 //   * accumulates the "own" halves  sum_j P_ij  and  -1/2 sum_j r_ij (x) P_ij  and U_i.
 // T = double (MD_FP64) or float (MD_FP32: r_ij formed in double, then rounded; reading A10).
+#include <algorithm>
 #include <cstdlib>
 
 #include "common.cuh"
@@ -25,7 +26,6 @@ struct TersoffDev {
 };
 
 constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom (generic path)
-constexpr int TERSOFF_MR = 6;    // list-row length handled by the register path
 
 // Generic path: any number of in-range neighbours up to TERSOFF_KC, per-thread arrays in local memory.
 // Used by threads whose list row is longer than the register path's MR slots.
@@ -168,35 +168,40 @@ __device__ __forceinline__ double min_image_listed(double d, double L, int hi_ha
 // (rare) cut-off window R < r < S.
 template <class T, class Rec, int MR, int MINB>
 __global__ void __launch_bounds__(128, MINB)
-k_tersoff_atom(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
                const double* __restrict__ z, double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                int* __restrict__ status) {
+    // Loads first, in two dependent levels only: {NN, NL, REV, math tables} -> {x[j]}.  The list slots are
+    // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
+    // index and masked out below), and the table staging's barrier comes after the loads are in flight.
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
-    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
-    __syncthreads();
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = i0 < n ? i0 : n - 1;
     const int nn = NN[i];
+    int jd[MR], rv[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) {
+        const int mk = m < K ? m : 0;
+        const int jr = NL[(int64_t)mk * n + i];
+        jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
+        rv[m] = (int)REV[(int64_t)mk * n + i];
+    }
+    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    const double xi = x[i], yi = y[i], zi = z[i];
+    double dx[MR], dy[MR], dz[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
+    __syncthreads();
+    if (i0 >= n) return;
     if (nn > MR) {
         tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, virial, status);
         return;
     }
-    const double xi = x[i], yi = y[i], zi = z[i];
     const int hhx = __double2hiint(0.5 * Lx), hhy = __double2hiint(0.5 * Ly), hhz = __double2hiint(0.5 * Lz);
-
-    int jd[MR], rv[MR];
-    double dx[MR], dy[MR], dz[MR];
-#pragma unroll
-    for (int m = 0; m < MR; ++m) {
-        jd[m] = m < nn ? NL[(int64_t)m * n + i] : (int)i;
-        rv[m] = m < nn ? (int)REV[(int64_t)m * n + i] : 0;
-    }
-#pragma unroll
-    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
 
     T ex[MR], ey[MR], ez[MR], rinv[MR], rr[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
     unsigned mask = 0u, window = 0u;
@@ -455,11 +460,11 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
 #define MD_TERSOFF_LAUNCH(MRV, MINB)                                                                      \
-    k_tersoff_atom<T, Rec, MRV, MINB><<<gb, 128, 0, s>>>(n, x, y, z, box[0], box[1], box[2], nl->NN,    \
+    k_tersoff_atom<T, Rec, MRV, MINB><<<gb, 128, 0, s>>>(n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN,    \
                                                          nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,          \
                                                          nl->MASK, pe, f, virial, nl->d_status)
     static int mr = -1;
-    if (mr < 0) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 4; }
+    if (mr == -1) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 43; }
     if (mr == 0) {
         constexpr int TA = 64, PC = 8 * TA;
         using Sm = TersoffSmem<T, TA, PC>;
@@ -492,10 +497,10 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
-                      double* heat, cudaStream_t s) {
+                      double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0) return MD_OK;
     int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, s)
                                   : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, s);
     if (rc != MD_OK) return rc;
-    return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, s);
+    return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, vv, s);
 }

@@ -236,6 +236,47 @@ def test_nve_energy_conservation_on_gpu(pot):
     assert 3.0 <= dev_e[0] / dev_e[1] <= 5.0, dev_e
 
 
+@pytest.mark.parametrize("pot", ["tersoff", "sw"])
+def test_nve_run_is_bitwise_the_composition_of_the_four_calls(pot):
+    """md_nve_run fuses the half-kicks into its gather kernel; the result must be bit for bit what the
+    public calls give when composed by hand: kick+drift, [build], force, kick."""
+    s = mi.silicon_crystal(3, 0.05, 300.0, 21)
+    K, P, rl = KMAX[pot], PARAMS[pot], mi.r_list(pot)
+    force = md.md_tersoff_force if pot == "tersoff" else md.md_sw_force
+    a, b = GpuSystem(s, K), GpuSystem(s, K)
+    n = a.n
+    fa = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+    fb = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+    pea = torch.zeros(n, dtype=torch.float64, device=DEV)
+    peb = torch.zeros(n, dtype=torch.float64, device=DEV)
+    nsteps, every, dt = 13, 5, 1.0
+    md.md_nve_run(a.nl, pot, P, n, a.x, a.y, a.z, a.vx, a.vy, a.vz, fa, False, pea, a.box, a.mass, dt, nsteps,
+                  every, rl)
+    md.md_build_neighbors(b.nl, n, b.x, b.y, b.z, b.box, rl)
+    force(b.nl, n, b.x, b.y, b.z, b.vx, b.vy, b.vz, b.box, P, f=fb)
+    for step in range(nsteps):
+        md.md_velocity_verlet_step(0, n, b.x, b.y, b.z, b.vx, b.vy, b.vz, fb, b.mass, dt, b.box)
+        if step % every == 0:
+            md.md_build_neighbors(b.nl, n, b.x, b.y, b.z, b.box, rl)
+        force(b.nl, n, b.x, b.y, b.z, b.vx, b.vy, b.vz, b.box, P, pe=peb, f=fb)
+        md.md_velocity_verlet_step(1, n, b.x, b.y, b.z, b.vx, b.vy, b.vz, fb, b.mass, dt, b.box)
+    md.md_neighbors_status(a.nl); md.md_neighbors_status(b.nl)
+    sa, sb = a.state(), b.state()
+    for k in ("x", "y", "z", "vx", "vy", "vz"):
+        assert (sa[k] == sb[k]).all(), k
+    assert (fa.cpu().numpy() == fb.cpu().numpy()).all()
+    assert (pea.cpu().numpy() == peb.cpu().numpy()).all()
+    # and continuing a run (f_valid = 1, first_step > 0) is the same as one long run
+    c = GpuSystem(s, K)
+    fc = torch.zeros((3, n), dtype=torch.float64, device=DEV)
+    md.md_nve_run(c.nl, pot, P, n, c.x, c.y, c.z, c.vx, c.vy, c.vz, fc, False, None, c.box, c.mass, dt, 6, every, rl)
+    md.md_nve_run(c.nl, pot, P, n, c.x, c.y, c.z, c.vx, c.vy, c.vz, fc, True, None, c.box, c.mass, dt, nsteps - 6,
+                  every, rl, first_step=6)
+    sc = c.state()
+    for k in ("x", "y", "z", "vx", "vy", "vz"):
+        assert (sa[k] == sc[k]).all(), k
+
+
 def test_nve_run_host_matches_device_run():
     s = mi.silicon_crystal(3, 0.05, 300.0, 15)
     g = GpuSystem(s, 16)
