@@ -56,7 +56,8 @@ __device__ __forceinline__ float rsqrt(float a) { return ::rsqrtf(a); }
 
 // exp(x): k = round(64 x / ln 2), r = x - k ln2/64 (two parts, |r| <= 0.00542), degree-5 Taylor
 // (truncation 3.5e-17), times 2^(j/64) from the table with k >> 6 added to its exponent field.
-// Saturates instead of overflowing: the exponent shift is clamped to +-1020.
+// Saturates instead of overflowing: the exponent shift is clamped to +-1020.  Domain |x| < 2e7
+// (k must fit an int32); callers with unbounded arguments clamp them first.
 __device__ __forceinline__ double exp(double x, const Tab& tb) {
     const double kd = __fma_rn(x, 92.33248261689366, 6755399441055744.0);     // 1.5 * 2^52
     const int k = __double2loint(kd);

@@ -130,10 +130,13 @@ __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double*
 }
 
 constexpr int SEARCH_BT = 128;
+#ifndef SEARCH_UNROLL
+#define SEARCH_UNROLL 2
+#endif
 
 __global__ void __launch_bounds__(SEARCH_BT)
 k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __restrict__ sortedf,
-         const int32_t* __restrict__ cell_start, int K, float rc2_screen, int32_t* __restrict__ NN,
+         const int32_t* __restrict__ cell_start, int K, float rc2_lo, float rc2_hi, int32_t* __restrict__ NN,
          int32_t* __restrict__ NL, int* __restrict__ status) {
     extern __shared__ int s_nb[];                            // [K][SEARCH_BT]: this thread's row, sorted
     const int tid = threadIdx.x;
@@ -146,60 +149,89 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
     const int cy = cell_coord(a.y, g.inv_cell[1], g.nc[1]);
     const int cz = cell_coord(a.z, g.inv_cell[2], g.nc[2]);
     const float Lxf = (float)g.L[0], Lyf = (float)g.L[1], Lzf = (float)g.L[2];
-    const bool interior_z = cz > 0 && cz < g.nc[2] - 1;
     int cnt = 0;
-    for (int ox = -1; ox <= 1; ++ox) {
-        int ax = cx + ox;
-        float xs = xf;                                       // reference shifted instead of the candidate
+
+    // One candidate.  The FP32 distance decides whenever it is outside the band [rc2_lo, rc2_hi) that its
+    // error bound leaves open (see md_launch_build); inside the band (about one candidate in 10^4) the
+    // canonical FP64 predicate of reading A7 decides, with explicit roundings and no contraction.  Either
+    // way the outcome is that predicate's.  A hit is appended with a predicated store (no divergent
+    // insertion inside the scan); the row is sorted once at the end.
+    auto test = [&](int q, const float4 bf, float xs, float ys, float zs) {
+        const float fx = bf.x - xs, fy = bf.y - ys, fz = bf.z - zs;
+        const float d2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+        const int j = __float_as_int(bf.w);
+        bool hit = d2f < rc2_hi && j != i;
+        if (hit && d2f >= rc2_lo) {
+            const double4 b = sorted[q];
+            const double dx = md_min_image(__dsub_rn(b.x, a.x), g.L[0], g.halfL[0]);
+            const double dy = md_min_image(__dsub_rn(b.y, a.y), g.L[1], g.halfL[1]);
+            const double dz = md_min_image(__dsub_rn(b.z, a.z), g.L[2], g.halfL[2]);
+            const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+            hit = d2 < g.rc2;
+        }
+        if (hit && cnt < K) s_nb[cnt * SEARCH_BT + tid] = j;
+        cnt += hit ? 1 : 0;
+    };
+    // a contiguous range of the cell-ordered array, SEARCH_UNROLL candidates in flight at a time
+    auto scan = [&](int beg, int end, float xs, float ys, float zs) {
+        const float4 far = make_float4(1e18f, 1e18f, 1e18f, __int_as_float(i));
+        for (int q = beg; q < end; q += SEARCH_UNROLL) {
+            float4 c[SEARCH_UNROLL];
+#pragma unroll
+            for (int u = 0; u < SEARCH_UNROLL; ++u) c[u] = (u == 0 || q + u < end) ? sortedf[q + u] : far;
+#pragma unroll
+            for (int u = 0; u < SEARCH_UNROLL; ++u) test(q + u, c[u], xs, ys, zs);
+        }
+    };
+
+    int axs[3], ays[3];
+    float xss[3], yss[3];
+#pragma unroll
+    for (int o = 0; o < 3; ++o) {                            // the reference is shifted, not the candidate
+        int ax = cx + o - 1; float xs = xf;
         if (ax < 0) { ax += g.nc[0]; xs += Lxf; } else if (ax >= g.nc[0]) { ax -= g.nc[0]; xs -= Lxf; }
-        for (int oy = -1; oy <= 1; ++oy) {
-            int ay = cy + oy;
-            float ys = yf;
-            if (ay < 0) { ay += g.nc[1]; ys += Lyf; } else if (ay >= g.nc[1]) { ay -= g.nc[1]; ys -= Lyf; }
-            const int base = (ax * g.nc[1] + ay) * g.nc[2];
-            // one contiguous range for an interior atom, else the three z cells one by one
-            const int nseg = interior_z ? 1 : 3;
-            for (int sg = 0; sg < nseg; ++sg) {
-                int beg, end;
-                float zs = zf;
-                if (interior_z) {
-                    beg = cell_start[base + cz - 1];
-                    end = cell_start[base + cz + 2];
-                } else {
-                    int az = cz + sg - 1;
-                    if (az < 0) { az += g.nc[2]; zs += Lzf; } else if (az >= g.nc[2]) { az -= g.nc[2]; zs -= Lzf; }
-                    beg = cell_start[base + az];
-                    end = cell_start[base + az + 1];
-                }
-                for (int q = beg; q < end; ++q) {
-                    const float4 bf = sortedf[q];
-                    const float fx = bf.x - xs, fy = bf.y - ys, fz = bf.z - zs;
-                    if (fmaf(fz, fz, fmaf(fy, fy, fx * fx)) >= rc2_screen) continue;    // FP32 screen
-                    const double4 b = sorted[q];
-                    const int j = (int)__double_as_longlong(b.w);
-                    // canonical predicate (reading A7): explicit roundings, no contraction
-                    const double dx = md_min_image(__dsub_rn(b.x, a.x), g.L[0], g.halfL[0]);
-                    const double dy = md_min_image(__dsub_rn(b.y, a.y), g.L[1], g.halfL[1]);
-                    const double dz = md_min_image(__dsub_rn(b.z, a.z), g.L[2], g.halfL[2]);
-                    const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-                    if (d2 < g.rc2 && j != i) {
-                        if (cnt < K) {
-                            int p = cnt;                      // insertion keeps the row sorted by j
-                            while (p > 0 && s_nb[(p - 1) * SEARCH_BT + tid] > j) {
-                                s_nb[p * SEARCH_BT + tid] = s_nb[(p - 1) * SEARCH_BT + tid];
-                                --p;
-                            }
-                            s_nb[p * SEARCH_BT + tid] = j;
-                        }
-                        ++cnt;
-                    }
-                }
+        int ay = cy + o - 1; float ys = yf;
+        if (ay < 0) { ay += g.nc[1]; ys += Lyf; } else if (ay >= g.nc[1]) { ay -= g.nc[1]; ys -= Lyf; }
+        axs[o] = ax; xss[o] = xs; ays[o] = ay; yss[o] = ys;
+    }
+    if (cz > 0 && cz < g.nc[2] - 1) {
+        // interior in z: the three z-neighbour cells of a column are contiguous in cell order, so the
+        // 27 cells are 9 ranges; all 18 bounds are fetched before the first scan
+        int beg[9], end[9];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+            const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * g.nc[2] + cz;
+            beg[c] = cell_start[base - 1];
+            end[c] = cell_start[base + 2];
+        }
+#pragma unroll
+        for (int c = 0; c < 9; ++c) scan(beg[c], end[c], xss[c / 3], yss[c % 3], zf);
+    } else {
+        for (int c = 0; c < 9; ++c) {
+            const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * g.nc[2];
+            for (int oz = -1; oz <= 1; ++oz) {
+                int az = cz + oz; float zs = zf;
+                if (az < 0) { az += g.nc[2]; zs += Lzf; } else if (az >= g.nc[2]) { az -= g.nc[2]; zs -= Lzf; }
+                scan(cell_start[base + az], cell_start[base + az + 1], xss[c / 3], yss[c % 3], zs);
             }
         }
     }
-    atomicMax(&status[1], cnt);
+    {   // longest row: one atomic per warp
+        const unsigned act = __activemask();
+        const int wmax = __reduce_max_sync(act, cnt);
+        if ((tid & 31) == __ffs(act) - 1) atomicMax(&status[1], wmax);
+    }
     if (cnt > K) { atomicOr(&status[0], MD_DEV_ROW_OVERFLOW); cnt = K; }
     NN[i] = cnt;
+    for (int m = 1; m < cnt; ++m) {                          // insertion sort of the (short) row by index
+        const int j = s_nb[m * SEARCH_BT + tid];
+        int p = m;
+        while (p > 0 && s_nb[(p - 1) * SEARCH_BT + tid] > j) {
+            s_nb[p * SEARCH_BT + tid] = s_nb[(p - 1) * SEARCH_BT + tid];
+            --p;
+        }
+        s_nb[p * SEARCH_BT + tid] = j;
+    }
     for (int m = 0; m < cnt; ++m) NL[(int64_t)m * n + i] = s_nb[m * SEARCH_BT + tid];
 }
 
@@ -267,13 +299,18 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     k_scan_add<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks, (int32_t)n);
     k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted,
                                  nl->sortedf);
-    // FP32 screen: float coordinates carry an absolute error <= 2^-24 max(L) each, so |d2_f32 - d2| is
-    // below 4 (r_list + e) e + rounding with e = 3 * 2^-23 max(L); the margin below is 4x that bound.
+    // FP32 screen.  A coordinate in [0, L) rounds to float within u = 2^-24 Lmax; the shifted reference
+    // x +- L carries at most 4u, so each float component differs from the canonical FP64 one by less than
+    // 5u (+ 1e-13 of FP64 rounding), and for a candidate near the cut-off |d2_f32 - d2| is below
+    // 2 sqrt(3) (r_list + 5u) 5u + 3 (5u)^2 + 2^-22 d2 < 18 (r_list + e) e with e = 6u.  The band
+    // [rc2 - m, rc2 + m) with m = 32 (r_list + e) e + 1e-6 rc2 is nearly twice that bound: outside it
+    // the float comparison and the FP64 predicate agree; inside it the FP64 predicate is evaluated.
     const double Lmax = fmax(box[0], fmax(box[1], box[2]));
-    const double e = 3.0 * Lmax * 1.1920929e-7;
-    const float rc2_screen = (float)(g.rc2 + 16.0 * (r_list + e) * e + 1e-6 * g.rc2);
+    const double e = 6.0 * Lmax * 5.9604645e-8;
+    const double band = 32.0 * (r_list + e) * e + 1e-6 * g.rc2;
+    const float rc2_lo = (float)(g.rc2 - band) , rc2_hi = (float)(g.rc2 + band);
     k_search<<<(unsigned)((n + SEARCH_BT - 1) / SEARCH_BT), SEARCH_BT, sizeof(int) * SEARCH_BT * nl->K, s>>>(
-        n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K, rc2_screen, nl->NN, nl->NL, nl->d_status);
+        n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K, rc2_lo, rc2_hi, nl->NN, nl->NL, nl->d_status);
     }
     MD_CUDA_TRY(cudaGetLastError());
     return md_launch_reverse(nl, s);

@@ -9,6 +9,8 @@
 // Same push / own-half scheme as tersoff.cu.
 #include "common.cuh"
 #include "real_math.cuh"
+#include "pair_cta.cuh"
+#include "fastmath.cuh"
 
 namespace {
 
@@ -18,104 +20,124 @@ struct SWDev {
     int ip, iq;      // integer exponents if p, q are small non-negative integers, else -1
 };
 
-constexpr int SW_KC = 32;
-
 template <class T> __device__ __forceinline__ T ipow(T a, int e) {
     T r = T(1);
     for (int k = 0; k < e; ++k) r *= a;
     return r;
 }
 
-template <class T, class Rec>
-__global__ void __launch_bounds__(128)
-k_sw_pair(int64_t n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
-          double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-          const uint8_t* __restrict__ REV, SWDev<T> p, Rec* __restrict__ Q,
-          unsigned long long* __restrict__ MASK, double* __restrict__ pe, double* __restrict__ f,
-          double* __restrict__ virial, int* __restrict__ status) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double xi = x[i], yi = y[i], zi = z[i];
-    const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
-    const int nn = NN[i];
+// "lanes = pairs" kernel.  The SW list holds the whole second shell (16-18 entries at the 0.5 A skin) but
+// only ~6 of them are inside r_c, so a thread-per-atom loop would idle most lanes and spill its per-
+// neighbour arrays.  A CTA of 256 threads owns TA atoms:
+//   stage A  compaction of the in-range pairs into shared memory              (pair_cta.cuh)
+//   stage B  per pair: e_ij, 1/r, V2, V2', s_j = exp(gamma sigma/(r - r_c)), ds_j
+//   stage C  per pair: three-body sums over the other in-range pairs of the same atom, P_ij pushed
+//            to Q[rev(i,m)*n + j]
+//   stage D  per atom: U_i, own halves sum_j P_ij and -1/2 sum_j r_ij (x) P_ij, MASK
+template <class T, int TA, int PC>
+struct SWSmem {
+    pc::Dense<T, TA, PC> d;
+    T rinv[PC], sj[PC], ds[PC], D[PC], Uh[PC];   // Uh: V2/2, then + the pair's share of the V3 terms
+    T Px[PC], Py[PC], Pz[PC];
+    __align__(16) double tab[fm::TAB_DOUBLES];
+};
 
-    T ex[SW_KC], ey[SW_KC], ez[SW_KC], rinv[SW_KC], sj[SW_KC], ds[SW_KC];
-    T Px[SW_KC], Py[SW_KC], Pz[SW_KC];
-    int jdx[SW_KC];
-    unsigned char slot[SW_KC];
-    int M = 0;
-    unsigned long long mask = 0ull;
-    T U = T(0);
+template <class T, class Rec, int TA, int PC>
+__global__ void __launch_bounds__(pc::NT)
+k_sw_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
+               const double* __restrict__ z, double Lx, double Ly, double Lz,
+               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+               const uint8_t* __restrict__ REV, SWDev<T> p, const double* __restrict__ gtab,
+               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+               int* __restrict__ status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SWSmem<T, TA, PC>& s = *reinterpret_cast<SWSmem<T, TA, PC>*>(smem_raw);
+    const int tid = threadIdx.x;
+    const int64_t A0 = (int64_t)blockIdx.x * TA;
+    const int na = (int)min((int64_t)TA, n - A0);
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after compact_in_range's barriers
+    pc::compact_in_range<T, TA, PC>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.rc2, status);
+    const int np = s.d.np;
 
-    for (int m = 0; m < nn; ++m) {
-        const int j = NL[(int64_t)m * n + i];
-        const double dx = md_min_image(x[j] - xi, Lx, hx);
-        const double dy = md_min_image(y[j] - yi, Ly, hy);
-        const double dz = md_min_image(z[j] - zi, Lz, hz);
-        const T tx = (T)dx, ty = (T)dy, tz = (T)dz;
+    // stage B
+    for (int k = tid; k < np; k += pc::NT) {
+        const T tx = s.d.ex[k], ty = s.d.ey[k], tz = s.d.ez[k];
         const T d2 = tx * tx + ty * ty + tz * tz;
-        if (d2 < p.rc2) {
-            const T ri = rm::rsqrt(d2);
-            const T rr = d2 * ri;
-            if (!(rr < p.rc)) continue;                     // never divide by r - r_c = 0 (reading A8)
-            if (M >= SW_KC) { atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); continue; }
-            const T e0 = tx * ri, e1 = ty * ri, e2 = tz * ri;
-            const T u = T(1) / (rr - p.rc);                 // < 0
-            // two-body: V2 = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - rc))
-            const T sr = p.sigma * ri;
-            const T sp = p.ip >= 0 ? ipow(sr, p.ip) : rm::pow(sr, p.p);
-            const T sq = p.iq >= 0 ? ipow(sr, p.iq) : rm::pow(sr, p.q);
-            const T ev = p.Aeps * rm::exp(p.sigma * u);
-            const T br = p.B * sp - sq;
-            const T V2 = ev * br;
-            const T V2p = ev * ((p.q * sq - p.p * p.B * sp) * ri - br * p.sigma * u * u);
-            U += T(0.5) * V2;
-            const T D = T(0.5) * V2p;
-            ex[M] = e0; ey[M] = e1; ez[M] = e2; rinv[M] = ri;
-            Px[M] = D * e0; Py[M] = D * e1; Pz[M] = D * e2;
-            sj[M] = rm::exp(p.gs * u);
-            ds[M] = -p.gs * u * u;
-            jdx[M] = j; slot[M] = (unsigned char)m;
-            mask |= 1ull << m;
-            ++M;
-        }
+        const T ri = fm::rsqrt(d2);
+        const T rr = d2 * ri;
+        s.d.ex[k] = tx * ri; s.d.ey[k] = ty * ri; s.d.ez[k] = tz * ri; s.rinv[k] = ri;
+        const bool ok = rr < p.rc;                          // never divide by r - r_c = 0 (reading A8)
+        // u = 1/(r - r_c) < 0, clamped at -300: beyond that exp(sigma u) < 1e-270 is zero for every purpose,
+        // and fm::exp wants |argument| < 2e7
+        const T u = ok ? max(fm::rcp(rr - p.rc), T(-300)) : T(-1);
+        // two-body: V2 = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - rc))
+        const T sr = p.sigma * ri;
+        const T sp = p.ip >= 0 ? ipow(sr, p.ip) : rm::pow(sr, p.p);
+        const T sq = p.iq >= 0 ? ipow(sr, p.iq) : rm::pow(sr, p.q);
+        const T ev = ok ? p.Aeps * fm::exp(p.sigma * u, tb) : T(0);
+        const T br = p.B * sp - sq;
+        s.Uh[k] = T(0.5) * ev * br;
+        s.D[k] = T(0.5) * ev * ((p.q * sq - p.p * p.B * sp) * ri - br * p.sigma * u * u);
+        s.sj[k] = ok ? fm::exp(p.gs * u, tb) : T(0);
+        s.ds[k] = -p.gs * u * u;
     }
+    __syncthreads();
 
-    for (int a = 0; a < M; ++a)
-        for (int b = a + 1; b < M; ++b) {
-            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+    // stage C: P_a = D_a e_a + sum_{b != a} E [ ds_a delta^2 e_a + 2 delta (e_b - cos e_a)/r_a ],
+    // E = lambda eps s_a s_b, delta = cos - cos0; V3 of a triplet belongs to the central atom (A6)
+    for (int k = tid; k < np; k += pc::NT) {
+        const int tmk = s.d.tm[k];
+        const int t = tmk >> 6, m = tmk & 63;
+        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
+        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
+        const T sa = p.leps * s.sj[k], dsa = s.ds[k], two_ria = T(2) * s.rinv[k];
+        T ce = s.D[k];                                       // coefficient of e_a
+        T sx = T(0), sy = T(0), sz = T(0), u3 = T(0);
+        for (int b = b0; b < b1; ++b) {
+            if (b == k) continue;
+            const T bx = s.d.ex[b], by = s.d.ey[b], bz = s.d.ez[b];
+            const T cs = ax * bx + ay * by + az * bz;
             const T dl = cs - p.cos0;
-            const T E = p.leps * sj[a] * sj[b];
-            const T Ed = E * dl;
-            U += Ed * dl;                                   // V3 belongs to the central atom i
-            const T ta = T(2) * Ed * rinv[a], tb = T(2) * Ed * rinv[b];
-            const T ua = Ed * dl * ds[a] - ta * cs;
-            const T ub = Ed * dl * ds[b] - tb * cs;
-            Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
-            Px[b] += tb * ex[a] + ub * ex[b]; Py[b] += tb * ey[a] + ub * ey[b]; Pz[b] += tb * ez[a] + ub * ez[b];
+            const T Ed = sa * s.sj[b] * dl;
+            const T Edd = Ed * dl;
+            u3 += Edd;
+            const T ta = Ed * two_ria;
+            ce += Edd * dsa - ta * cs;
+            sx += ta * bx; sy += ta * by; sz += ta * bz;
         }
-
-    T Fx = T(0), Fy = T(0), Fz = T(0);
-    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
-    for (int a = 0; a < M; ++a) {
-        const int m = slot[a];
+        const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
+        s.Px[k] = px; s.Py[k] = py; s.Pz[k] = pz;
+        s.Uh[k] += T(0.5) * u3;                              // each unordered pair (a,b) is met twice
+        const int64_t i = A0 + t;
         const int mm = REV[(int64_t)m * n + i];
-        rm::store_rec(&Q[(int64_t)mm * n + jdx[a]], Px[a], Py[a], Pz[a]);
-        Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
-        if (virial) {
-            const T rr = T(1) / rinv[a];
-            const T rx = ex[a] * rr, ry = ey[a] * rr, rz = ez[a] * rr;
-            W[0] += rx * Px[a]; W[1] += rx * Py[a]; W[2] += rx * Pz[a];
-            W[3] += ry * Px[a]; W[4] += ry * Py[a]; W[5] += ry * Pz[a];
-            W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
-        }
+        rm::store_rec(&Q[(int64_t)mm * n + s.d.j[k]], px, py, pz);
     }
-    MASK[i] = mask;
-    if (pe) pe[i] = (double)U;
-    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
-    if (virial) {
+    __syncthreads();
+
+    // stage D: per-atom sums
+    for (int t = tid; t < na; t += pc::NT) {
+        const int64_t i = A0 + t;
+        T U = T(0), Fx = T(0), Fy = T(0), Fz = T(0);
+        T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+        for (int b = s.d.off[t]; b < s.d.off[t + 1]; ++b) {
+            const T px = s.Px[b], py = s.Py[b], pz = s.Pz[b];
+            U += s.Uh[b]; Fx += px; Fy += py; Fz += pz;
+            if (virial) {
+                const T rr = T(1) / s.rinv[b];
+                const T rx = s.d.ex[b] * rr, ry = s.d.ey[b] * rr, rz = s.d.ez[b] * rr;
+                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+            }
+        }
+        MASK[i] = s.d.mask[t];
+        if (pe) pe[i] = (double)U;
+        if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+        if (virial) {
 #pragma unroll
-        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+            for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+        }
     }
 }
 
@@ -133,9 +155,19 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.rc = (T)rc; p.rc2 = (T)(rc * rc); p.gs = (T)(hp->gamma * hp->sigma);
     p.leps = (T)(hp->lambda * hp->epsilon); p.cos0 = (T)hp->cos0; p.p = (T)hp->p; p.q = (T)hp->q;
     p.ip = small_int(hp->p); p.iq = small_int(hp->q);
+    const double* gtab = md_math_tables();
+    if (!gtab) return MD_ERR_ALLOC;
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
-    k_sw_pair<T, Rec><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(
-        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
+    constexpr int TA = 40, PC = 16 * TA;                     // ~6 in-range pairs per atom: ~240 per CTA
+    using Sm = SWSmem<T, TA, PC>;
+    auto kern = k_sw_pairs_cta<T, Rec, TA, PC>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        MD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Sm)));
+        attr_set = true;
+    }
+    kern<<<(unsigned)((n + TA - 1) / TA), pc::NT, sizeof(Sm), s>>>(
+        n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
         pe, f, virial, nl->d_status);
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
