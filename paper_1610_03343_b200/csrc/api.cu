@@ -12,6 +12,8 @@ void free_all(md_neighbors* nl) {
     cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e);
+    if (nl->h_maxrow) cudaFreeHost(nl->h_maxrow);
+    if (nl->ev_list) cudaEventDestroy(nl->ev_list);
     if (nl->ev_pool) for (cudaEvent_t e : *nl->ev_pool) cudaEventDestroy(e);
     delete nl->ev_pool; delete nl->ev_kind;
 }
@@ -58,6 +60,15 @@ ProfScope::ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_) : nl(
     on = true;
 }
 ProfScope::~ProfScope() { if (on) cudaEventRecord(e1, s); }
+
+int md_list_max_row(md_neighbors* nl, int* max_row) {
+    if (nl->maxrow_pending) {
+        MD_CUDA_TRY(cudaEventSynchronize(nl->ev_list));
+        nl->maxrow_pending = 0;
+    }
+    *max_row = *nl->h_maxrow;
+    return MD_OK;
+}
 
 extern "C" {
 
@@ -114,6 +125,8 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sortedf, n * sizeof(float4)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->d_status, 2 * sizeof(int)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&nl->h_maxrow, sizeof(int)) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&nl->ev_list, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { cudaGetLastError(); free_all(nl); delete nl; return MD_ERR_ALLOC; }
     cudaMemset(nl->d_status, 0, 2 * sizeof(int));
     *out = nl;
@@ -155,6 +168,7 @@ int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const in
     cudaStream_t s = (cudaStream_t)stream;
     nl->n = n;
     if (n == 0) return MD_OK;
+    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, sizeof(int), s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NN, NN, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NL, NL, sizeof(int32_t) * n * nl->K, cudaMemcpyDeviceToDevice, s));
     return md_launch_reverse(nl, s);

@@ -463,8 +463,17 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     k_tersoff_atom<T, Rec, MRV, MINB><<<gb, 128, 0, s>>>(n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN,    \
                                                          nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,          \
                                                          nl->MASK, pe, f, virial, nl->d_status)
-    static int mr = -1;
-    if (mr == -1) { const char* e = getenv("MD_TERSOFF_MR"); mr = e ? atoi(e) : 43; }
+    // Kernel selection by the longest row of the list (known on the host once per build): rows of up to
+    // 4 entries (the crystal) take the register kernel; longer rows the lanes = pairs CTA kernel.
+    static int forced = -1;
+    if (forced == -1) { const char* e = getenv("MD_TERSOFF_MR"); forced = e ? atoi(e) : -2; }
+    int mr = forced;
+    if (mr == -2) {
+        int max_row = 0;
+        const int rc = md_list_max_row(nl, &max_row);
+        if (rc != MD_OK) return rc;
+        mr = max_row <= 4 ? 43 : 0;
+    }
     if (mr == 0) {
         constexpr int TA = 64, PC = 8 * TA;
         using Sm = TersoffSmem<T, TA, PC>;
