@@ -256,7 +256,8 @@ def main_ours(args):
     n_pair = max(1, launches_prof["pair"])
     pair_ms = kinds_ms["pair"] / n_pair
     achieved = PAIR_FLOP_PER_ATOM[pot] * n / (pair_ms * 1e-3) / 1e12
-    kern = "k_tersoff_pair" if pot == "tersoff" else "k_sw_pair"
+    _, long_rows = md.md_neighbors_row_stats(nl)
+    kern = "k_sw_pairs_cta" if pot == "sw" else ("k_tersoff_pairs_cta" if long_rows * 256 > n else "k_tersoff_atom")
     value = world * n * args.steps / (ms_total * 1e-3)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -68,6 +68,12 @@ int md_neighbors_destroy(md_neighbors* nl);
  * max_count_seen (HOST, may be NULL) receives the longest row of the last build. */
 int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream);
 
+/* Row statistics of the current list (HOST ints, either may be NULL): the longest row and the number
+ * of rows longer than 4 entries.  Waits for the last build / import on its stream to finish.  The
+ * Tersoff call uses them to choose its kernel: the register kernel (k_tersoff_atom) while at most one
+ * row in 256 is longer than 4, else the lanes = pairs kernel (k_tersoff_pairs_cta). */
+int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than_4);
+
 /* Copy the current list out / in (DEVICE int32 buffers): NN[n]; NL[max_neighbors][n] neighbour-major,
  * NL[m*n + i] = index of the m-th neighbour of atom i, rows sorted by index.
  * Import also rebuilds the reverse index; it lets a test drive the force kernels with an

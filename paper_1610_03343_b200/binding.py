@@ -39,7 +39,7 @@ class md_sw_params(C.Structure):
 EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neighbors_status",
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
-           "md_profile_enable", "md_profile_read", "md_math_probe")
+           "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats")
 
 _lib = None
 
@@ -186,6 +186,13 @@ def _pot(potential, params):
     if potential in (MD_SW, "sw"):
         return MD_SW, sw_params(params)
     raise MDError(MD_ERR_ARG, "potential")
+
+
+def md_neighbors_row_stats(nl):
+    """(longest row, rows longer than 4) of the current list."""
+    a, b = C.c_int(0), C.c_int(0)
+    _check(load().md_neighbors_row_stats(nl._h, C.byref(a), C.byref(b)), "md_neighbors_row_stats")
+    return a.value, b.value
 
 
 def md_nve_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, pe, box, mass_amu, dt_fs,

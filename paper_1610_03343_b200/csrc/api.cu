@@ -61,12 +61,13 @@ ProfScope::ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_) : nl(
 }
 ProfScope::~ProfScope() { if (on) cudaEventRecord(e1, s); }
 
-int md_list_max_row(md_neighbors* nl, int* max_row) {
+int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows) {
     if (nl->maxrow_pending) {
         MD_CUDA_TRY(cudaEventSynchronize(nl->ev_list));
         nl->maxrow_pending = 0;
     }
-    *max_row = *nl->h_maxrow;
+    *max_row = nl->h_maxrow[0];
+    *long_rows = nl->h_maxrow[1];
     return MD_OK;
 }
 
@@ -124,11 +125,11 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->rank_in_cell, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sortedf, n * sizeof(float4)) == cudaSuccess;
-    ok = ok && cudaMalloc(&nl->d_status, 2 * sizeof(int)) == cudaSuccess;
-    ok = ok && cudaMallocHost(&nl->h_maxrow, sizeof(int)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->d_status, 3 * sizeof(int)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&nl->h_maxrow, 2 * sizeof(int)) == cudaSuccess;
     ok = ok && cudaEventCreateWithFlags(&nl->ev_list, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { cudaGetLastError(); free_all(nl); delete nl; return MD_ERR_ALLOC; }
-    cudaMemset(nl->d_status, 0, 2 * sizeof(int));
+    cudaMemset(nl->d_status, 0, 3 * sizeof(int));
     *out = nl;
     return MD_OK;
 }
@@ -154,6 +155,17 @@ int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream) {
     return MD_OK;
 }
 
+int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than_4) {
+    if (!nl) return MD_ERR_ARG;
+    if (nl->n == 0) return MD_ERR_NO_LIST;
+    int a = 0, b = 0;
+    const int rc = md_list_row_stats(nl, &a, &b);
+    if (rc != MD_OK) return rc;
+    if (max_row) *max_row = a;
+    if (rows_longer_than_4) *rows_longer_than_4 = b;
+    return MD_OK;
+}
+
 int md_neighbors_export(md_neighbors* nl, int32_t* NN, int32_t* NL, void* stream) {
     if (!nl || !NN || !NL) return MD_ERR_ARG;
     if (nl->n == 0) return MD_OK;
@@ -168,7 +180,7 @@ int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const in
     cudaStream_t s = (cudaStream_t)stream;
     nl->n = n;
     if (n == 0) return MD_OK;
-    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, sizeof(int), s));
+    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, 2 * sizeof(int), s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NN, NN, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NL, NL, sizeof(int32_t) * n * nl->K, cudaMemcpyDeviceToDevice, s));
     return md_launch_reverse(nl, s);
@@ -179,7 +191,7 @@ int md_build_neighbors(md_neighbors* nl, int64_t n, const double* x, const doubl
     if (!nl || n < 0 || n > nl->n_cap || !valid_box(box) || !(r_list > 0)) return MD_ERR_ARG;
     if (n > 0 && (!x || !y || !z)) return MD_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
-    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, sizeof(int), s));
+    MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, 2 * sizeof(int), s));
     return md_launch_build(nl, n, x, y, z, box, r_list, s);
 }
 

@@ -46,10 +46,10 @@ struct md_neighbors {
     float4* sortedf;        // [n] the same in float (FP32 screen of the candidate search)
     int32_t* scan_blocks;   // block sums scratch
     // status
-    int* d_status;          // [2]: status bits, max row length seen
+    int* d_status;          // [3]: status bits, max row length seen, number of rows longer than 4
     // longest row of the current list, mirrored to the host for kernel selection: written by an async
     // copy at the end of every build / import; the first force call after it waits on the event
-    int* h_maxrow;          // pinned
+    int* h_maxrow;          // pinned [2]: longest row, number of rows longer than 4
     cudaEvent_t ev_list;
     int maxrow_pending;
     // profiling (md_profile_*)
@@ -98,7 +98,7 @@ struct ProfScope {
 int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                     const double box[3], double r_list, cudaStream_t s);
 int md_launch_reverse(md_neighbors* nl, cudaStream_t s);
-int md_list_max_row(md_neighbors* nl, int* max_row);   // host value of the longest row (may wait for the build)
+int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows);   // host copies (may wait for the build)
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,

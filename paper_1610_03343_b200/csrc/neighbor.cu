@@ -243,7 +243,11 @@ __global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, cons
     {   // longest row (also for imported lists): one atomic per warp
         const unsigned act = __activemask();
         const int wmax = __reduce_max_sync(act, nn);
-        if ((threadIdx.x & 31) == __ffs(act) - 1) atomicMax(&status[1], wmax);
+        const int nlong = __popc(__ballot_sync(act, nn > 4));
+        if ((threadIdx.x & 31) == __ffs(act) - 1) {
+            atomicMax(&status[1], wmax);
+            if (nlong) atomicAdd(&status[2], nlong);
+        }
     }
     for (int m = 0; m < nn; ++m) {
         const int j = NL[(int64_t)m * n + i];
@@ -264,7 +268,7 @@ int md_launch_reverse(md_neighbors* nl, cudaStream_t s) {
     ProfScope prof(nl, MD_KIND_BUILD, 1, s);
     k_reverse<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
     MD_CUDA_TRY(cudaGetLastError());
-    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_maxrow, nl->d_status + 1, sizeof(int), cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_maxrow, nl->d_status + 1, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     MD_CUDA_TRY(cudaEventRecord(nl->ev_list, s));
     nl->maxrow_pending = 1;
     return MD_OK;

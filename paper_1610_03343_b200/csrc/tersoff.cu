@@ -166,8 +166,8 @@ __device__ __forceinline__ double min_image_listed(double d, double L, int hi_ha
 // all MR slots, so ptxas interleaves the slots' independent FP64 chains; a slot that is empty or outside
 // the force range carries f_C = f_C' = f_R = f_A = 0 and drops out of every sum.  The only branch is the
 // (rare) cut-off window R < r < S.
-template <class T, class Rec, int MR, int MINB>
-__global__ void __launch_bounds__(128, MINB)
+template <class T, class Rec, int MR, int BT, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
 k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
                const double* __restrict__ z, double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
@@ -323,6 +323,7 @@ struct TersoffSmem {
     pc::Dense<T, TA, PC> d;
     T rinv[PC], fc[PC], fcp[PC], fRD[PC], fAu[PC], hh[PC];   // fRD: f_R then D; fAu: f_A then U_ij/2
     T Px[PC], Py[PC], Pz[PC];
+    __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
 template <class T, class Rec, int TA, int PC>
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(pc::NT)
 k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
                     const double* __restrict__ z, double Lx, double Ly, double Lz,
                     const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                    const uint8_t* __restrict__ REV, TersoffDev<T> p,
+                    const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
                     Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                     double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                     int* __restrict__ status) {
@@ -339,6 +340,7 @@ k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double
     const int tid = threadIdx.x;
     const int64_t A0 = (int64_t)blockIdx.x * TA;
     const int na = (int)min((int64_t)TA, n - A0);
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after compact_in_range's barriers
     pc::compact_in_range<T, TA, PC>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.S2, status);
     const int np = s.d.np;
 
@@ -346,19 +348,19 @@ k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double
     for (int k = tid; k < np; k += pc::NT) {
         const T tx = s.d.ex[k], ty = s.d.ey[k], tz = s.d.ez[k];
         const T d2 = tx * tx + ty * ty + tz * tz;
-        const T ri = rm::rsqrt(d2);
+        const T ri = fm::rsqrt(d2);
         const T rr = d2 * ri;
         s.d.ex[k] = tx * ri; s.d.ey[k] = ty * ri; s.d.ez[k] = tz * ri; s.rinv[k] = ri;
         T c = T(1), cp = T(0);
         if (rr > p.R) {                                      // f_C window R < r < S (reading A1)
             T sn, cs;
-            rm::sincos((rr - p.R) * p.w, &sn, &cs);
+            fm::sincos_0_pi((rr - p.R) * p.w, &sn, &cs);
             c = T(0.5) + T(0.5) * cs;
             cp = T(-0.5) * p.w * sn;
         }
         s.fc[k] = c; s.fcp[k] = cp;
-        s.fRD[k] = p.A * rm::exp(-p.lambda * rr);
-        s.fAu[k] = p.B * rm::exp(-p.mu * rr);
+        s.fRD[k] = p.A * fm::exp(-p.lambda * rr, tb);
+        s.fAu[k] = p.B * fm::exp(-p.mu * rr, tb);
     }
     __syncthreads();
 
@@ -373,13 +375,13 @@ k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double
             const T cs = ax * s.d.ex[b] + ay * s.d.ey[b] + az * s.d.ez[b];
             const T xx = p.h - cs;
             const T x2 = xx * xx;
-            zt += s.fc[b] * (T(1) + p.c2_over_d2 * x2 * pc::fast_rcp(p.d2 + x2));
+            zt += s.fc[b] * (T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2));
         }
         T bo = T(1), bp = T(0);
         if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
-            const T tt = rm::exp(p.n * rm::log(p.beta * zt));           // (beta zeta)^n
-            bo = rm::exp(p.minus_half_over_n * rm::log1p(tt));          // Eq. (3)
-            bp = T(-0.5) * bo * tt * pc::fast_rcp(zt * (T(1) + tt));
+            const T tt = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);               // (beta zeta)^n
+            bo = fm::exp(p.minus_half_over_n * fm::log(T(1) + tt, tb), tb);         // Eq. (3)
+            bp = T(-0.5) * bo * tt * fm::rcp(zt * (T(1) + tt));
         }
         const T c = s.fc[k], cp = s.fcp[k], fR = s.fRD[k], fA = s.fAu[k];
         const T bfA = bo * fA;
@@ -404,7 +406,7 @@ k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double
             const T cs = ax * bx + ay * by + az * bz;
             const T xx = p.h - cs;
             const T x2 = xx * xx;
-            const T q = pc::fast_rcp(p.d2 + x2);
+            const T q = fm::rcp(p.d2 + x2);
             const T hb = s.hh[b];
             const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
             const T ta = (ha * s.fc[b] + hb * ca) * gp * ria;
@@ -456,25 +458,20 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.w = (T)(3.14159265358979323846 / (hp->S - hp->R));
     p.minus_half_over_n = (T)(-0.5 / hp->n);
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
-    const unsigned gb = (unsigned)((n + 127) / 128);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
-#define MD_TERSOFF_LAUNCH(MRV, MINB)                                                                      \
-    k_tersoff_atom<T, Rec, MRV, MINB><<<gb, 128, 0, s>>>(n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN,    \
+#define MD_TERSOFF_LAUNCH(MRV, BT, MAXREG)                                                                 \
+    k_tersoff_atom<T, Rec, MRV, BT, MAXREG><<<(unsigned)((n + BT - 1) / BT), BT, 0, s>>>(n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN,    \
                                                          nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,          \
                                                          nl->MASK, pe, f, virial, nl->d_status)
-    // Kernel selection by the longest row of the list (known on the host once per build): rows of up to
-    // 4 entries (the crystal) take the register kernel; longer rows the lanes = pairs CTA kernel.
-    static int forced = -1;
-    if (forced == -1) { const char* e = getenv("MD_TERSOFF_MR"); forced = e ? atoi(e) : -2; }
-    int mr = forced;
-    if (mr == -2) {
-        int max_row = 0;
-        const int rc = md_list_max_row(nl, &max_row);
-        if (rc != MD_OK) return rc;
-        mr = max_row <= 4 ? 43 : 0;
-    }
-    if (mr == 0) {
+    // Kernel selection by the row lengths of the list (known on the host once per build): the register
+    // kernel handles rows of up to 4 entries (the crystal) in its fast path and longer ones through a slow
+    // per-thread fallback, so it is used while fewer than 1 row in 256 is longer; otherwise the
+    // lanes = pairs CTA kernel, whose cost does not depend on the row length.
+    int max_row = 0, long_rows = 0;
+    const int rcs = md_list_row_stats(nl, &max_row, &long_rows);
+    if (rcs != MD_OK) return rcs;
+    if ((int64_t)long_rows * 256 > n) {
         constexpr int TA = 64, PC = 8 * TA;
         using Sm = TersoffSmem<T, TA, PC>;
         auto kern = k_tersoff_pairs_cta<T, Rec, TA, PC>;
@@ -484,18 +481,12 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
             attr_set = true;
         }
         kern<<<(unsigned)((n + TA - 1) / TA), pc::NT, sizeof(Sm), s>>>(
-            n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, (Rec*)nl->Q, nl->MASK,
+            n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
             pe, f, virial, nl->d_status);
         MD_CUDA_TRY(cudaGetLastError());
         return MD_OK;
     }
-    switch (mr) {
-        case 43: MD_TERSOFF_LAUNCH(4, 3); break;
-        case 45: MD_TERSOFF_LAUNCH(4, 5); break;
-        case 5: MD_TERSOFF_LAUNCH(5, 3); break;
-        case 6: MD_TERSOFF_LAUNCH(6, 2); break;
-        default: MD_TERSOFF_LAUNCH(4, 4); break;
-    }
+    MD_TERSOFF_LAUNCH(4, 128, 168);
 #undef MD_TERSOFF_LAUNCH
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
