@@ -26,35 +26,56 @@ struct Dense {                   // shared-memory image of the CTA's in-range pa
 };
 
 // Stage A.  Returns after a __syncthreads(); d.np = number of dense pairs (clamped to PC).
-template <class T, int TA, int PC>
+// A task is one (slot m, atom t) of the CTA's list rows; consecutive threads take consecutive atoms, so a
+// warp reads 128 contiguous bytes of a list row.  Each thread owns up to TPT tasks and keeps their geometry
+// in registers: all its list entries are fetched first, then all neighbour coordinates (two dependent
+// memory levels for the whole stage, not two per task), and the dense entries are written from registers
+// once the prefix sum has placed them.  KL = longest list row the CTA can hold (rows beyond it latch
+// MD_DEV_INRANGE_OVERFLOW).
+template <class T, int TA, int PC, int KL>
 __device__ __forceinline__ void
 compact_in_range(Dense<T, TA, PC>& d, int64_t A0, int na, int64_t n, int K,
                  const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
                  double Lx, double Ly, double Lz, const int32_t* __restrict__ NN,
                  const int32_t* __restrict__ NL, T range2, int* __restrict__ status) {
+    constexpr int TPT = (KL * TA + NT - 1) / NT;
     const int tid = threadIdx.x;
     const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
     for (int t = tid; t < TA; t += NT) {
         d.mask[t] = 0ull;
-        d.nn[t] = t < na ? NN[A0 + t] : 0;
+        const int nn = t < na ? NN[A0 + t] : 0;
+        if (nn > KL) atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW);
+        d.nn[t] = nn < KL ? nn : KL;
     }
     __syncthreads();
-    // A1: one task per (slot m, atom t); consecutive threads -> consecutive atoms (coalesced NL rows)
-    int kmax = 0;
-    for (int t = 0; t < TA; ++t) kmax = max(kmax, d.nn[t]);          // smem broadcast reads
-    for (int q = tid; q < kmax * TA; q += NT) {
+    int jj[TPT];
+    T tx[TPT], ty[TPT], tz[TPT];
+    bool in[TPT];
+#pragma unroll
+    for (int u = 0; u < TPT; ++u) {                          // level 1: list entries
+        const int q = tid + u * NT;
         const int m = q / TA, t = q - m * TA;
-        if (m < d.nn[t]) {
-            const int64_t i = A0 + t;
-            const int jj = NL[(int64_t)m * n + i];
-            const T tx = (T)md_min_image(x[jj] - x[i], Lx, hx);
-            const T ty = (T)md_min_image(y[jj] - y[i], Ly, hy);
-            const T tz = (T)md_min_image(z[jj] - z[i], Lz, hz);
-            if (tx * tx + ty * ty + tz * tz < range2) atomicOr(&d.mask[t], 1ull << m);
-        }
+        in[u] = m < KL && m < d.nn[t];
+        jj[u] = in[u] ? NL[(int64_t)m * n + A0 + t] : (int)(A0 + t);
+    }
+#pragma unroll
+    for (int u = 0; u < TPT; ++u) {                          // level 2: coordinates
+        const int q = tid + u * NT;
+        const int t = q % TA;
+        const int64_t i = A0 + (t < na ? t : 0);
+        tx[u] = (T)md_min_image(x[jj[u]] - x[i], Lx, hx);
+        ty[u] = (T)md_min_image(y[jj[u]] - y[i], Ly, hy);
+        tz[u] = (T)md_min_image(z[jj[u]] - z[i], Lz, hz);
+    }
+#pragma unroll
+    for (int u = 0; u < TPT; ++u) {
+        const int q = tid + u * NT;
+        const int m = q / TA, t = q - m * TA;
+        in[u] = in[u] && tx[u] * tx[u] + ty[u] * ty[u] + tz[u] * tz[u] < range2;
+        if (in[u]) atomicOr(&d.mask[t], 1ull << m);
     }
     __syncthreads();
-    // A2: exclusive scan of the per-atom counts (TA <= NT)
+    // exclusive scan of the per-atom counts (TA <= NT)
     {
         const int c = tid < TA ? __popcll(d.mask[tid]) : 0;
         int inc = c;
@@ -86,21 +107,17 @@ compact_in_range(Dense<T, TA, PC>& d, int64_t A0, int na, int64_t n, int K,
         }
     }
     __syncthreads();
-    // A3: write the dense entries (geometry recomputed: L1-resident)
-    for (int q = tid; q < kmax * TA; q += NT) {
+    // dense entries, from registers
+#pragma unroll
+    for (int u = 0; u < TPT; ++u) {
+        if (!in[u]) continue;
+        const int q = tid + u * NT;
         const int m = q / TA, t = q - m * TA;
-        const unsigned long long mk = d.mask[t];
-        if (mk >> m & 1ull) {
-            const int k = d.off[t] + __popcll(mk & ((1ull << m) - 1ull));
-            if (k < PC) {
-                const int64_t i = A0 + t;
-                const int jj = NL[(int64_t)m * n + i];
-                d.j[k] = jj;
-                d.tm[k] = (unsigned short)(t * 64 + m);
-                d.ex[k] = (T)md_min_image(x[jj] - x[i], Lx, hx);
-                d.ey[k] = (T)md_min_image(y[jj] - y[i], Ly, hy);
-                d.ez[k] = (T)md_min_image(z[jj] - z[i], Lz, hz);
-            }
+        const int k = d.off[t] + __popcll(d.mask[t] & ((1ull << m) - 1ull));
+        if (k < PC) {
+            d.j[k] = jj[u];
+            d.tm[k] = (unsigned short)(t * 64 + m);
+            d.ex[k] = tx[u]; d.ey[k] = ty[u]; d.ez[k] = tz[u];
         }
     }
     __syncthreads();

@@ -57,7 +57,7 @@ k_sw_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __r
     const int64_t A0 = (int64_t)blockIdx.x * TA;
     const int na = (int)min((int64_t)TA, n - A0);
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after compact_in_range's barriers
-    pc::compact_in_range<T, TA, PC>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.rc2, status);
+    pc::compact_in_range<T, TA, PC, 32>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.rc2, status);
     const int np = s.d.np;
 
     // stage B
