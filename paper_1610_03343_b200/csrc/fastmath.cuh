@@ -129,4 +129,127 @@ __device__ __forceinline__ void sincos_0_pi(double a, double* sn, double* cs) {
 }
 __device__ __forceinline__ void sincos_0_pi(float a, float* sn, float* cs) { ::sincosf(a, sn, cs); }
 
+// ---- N independent evaluations, written stage by stage ---------------------------------------------------
+// ptxas schedules a chain of dependent FP64 instructions back to back if the source presents it that way
+// (a dependent DFMA issues every 8 cycles, an independent one every 2: measured).  The thread-per-atom
+// kernel has N = 4..8 independent evaluations at every step of its arithmetic (one per neighbour slot);
+// these versions advance all N together, one polynomial step at a time, so consecutive instructions in
+// the emitted order are independent.
+template <int N>
+__device__ __forceinline__ void exp_v(const double (&x)[N], double (&out)[N], const Tab& tb) {
+    double kd[N], kf[N], r[N], p[N], t[N];
+    int k[N];
+#pragma unroll
+    for (int m = 0; m < N; ++m) kd[m] = __fma_rn(x[m], 92.33248261689366, 6755399441055744.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) { k[m] = __double2loint(kd[m]); t[m] = tb.e[k[m] & (EXP_N - 1)]; }
+#pragma unroll
+    for (int m = 0; m < N; ++m) kf[m] = kd[m] - 6755399441055744.0;
+#pragma unroll
+    for (int m = 0; m < N; ++m) r[m] = __fma_rn(kf[m], -0.01083042469326756, x[m]);
+#pragma unroll
+    for (int m = 0; m < N; ++m) r[m] = __fma_rn(kf[m], -2.9815858269852933e-12, r[m]);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(r[m], 0.008333333333333333, 0.041666666666666664);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 0.16666666666666666);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 0.5);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 1.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 1.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+        const int sh = max(-1020, min(1020, k[m] >> 6));
+        out[m] = __hiloint2double(__double2hiint(t[m]) + (sh << 20), __double2loint(t[m])) * p[m];
+    }
+}
+template <int N>
+__device__ __forceinline__ void exp_v(const float (&x)[N], float (&out)[N], const Tab&) {
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = ::expf(x[m]);
+}
+
+template <int N>
+__device__ __forceinline__ void log_v(const double (&a)[N], double (&out)[N], const Tab& tb) {
+    double mm[N], r[N], p[N], ed[N], cy[N];
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+        const int hi = __double2hiint(a[m]), lo = __double2loint(a[m]);
+        const int e = (hi >> 20) - 1023;
+        const double2 cl = tb.l[(hi >> 14) & (LOG_N - 1)];
+        mm[m] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
+        ed[m] = __hiloint2double(0x43300000, e ^ 0x80000000);
+        r[m] = cl.x; cy[m] = cl.y;
+    }
+#pragma unroll
+    for (int m = 0; m < N; ++m) r[m] = __fma_rn(mm[m], r[m], -1.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) ed[m] = ed[m] - 4503601774854144.0;
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(r[m], 0.14285714285714285, -0.16666666666666666);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 0.2);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], -0.25);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], 0.3333333333333333);
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], r[m], -0.5);
+#pragma unroll
+    for (int m = 0; m < N; ++m) cy[m] = __fma_rn(ed[m], 0.6931471805599453, cy[m]);
+#pragma unroll
+    for (int m = 0; m < N; ++m) mm[m] = r[m] * r[m];
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = __fma_rn(p[m], mm[m], r[m]);
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = cy[m] + p[m];
+}
+template <int N>
+__device__ __forceinline__ void log_v(const float (&a)[N], float (&out)[N], const Tab&) {
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = ::logf(a[m]);
+}
+
+template <int N>
+__device__ __forceinline__ void rcp_v(const double (&a)[N], double (&out)[N]) {
+    double y[N], e[N];
+#pragma unroll
+    for (int m = 0; m < N; ++m) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y[m]) : "d"(a[m]));
+#pragma unroll
+    for (int m = 0; m < N; ++m) e[m] = __fma_rn(-a[m], y[m], 1.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) e[m] = __fma_rn(e[m], e[m], e[m]);
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = __fma_rn(y[m], e[m], y[m]);
+}
+template <int N>
+__device__ __forceinline__ void rcp_v(const float (&a)[N], float (&out)[N]) {
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = __frcp_rn(a[m]);
+}
+
+template <int N>
+__device__ __forceinline__ void rsqrt_v(const double (&a)[N], double (&out)[N]) {
+    double y[N], e[N], ay[N];
+#pragma unroll
+    for (int m = 0; m < N; ++m) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[m]) : "d"(a[m]));
+#pragma unroll
+    for (int m = 0; m < N; ++m) ay[m] = a[m] * y[m];
+#pragma unroll
+    for (int m = 0; m < N; ++m) e[m] = __fma_rn(-ay[m], y[m], 1.0);
+#pragma unroll
+    for (int m = 0; m < N; ++m) ay[m] = __fma_rn(e[m], 0.375, 0.5);
+#pragma unroll
+    for (int m = 0; m < N; ++m) e[m] = ay[m] * e[m];
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = __fma_rn(y[m], e[m], y[m]);
+}
+template <int N>
+__device__ __forceinline__ void rsqrt_v(const float (&a)[N], float (&out)[N]) {
+#pragma unroll
+    for (int m = 0; m < N; ++m) out[m] = ::rsqrtf(a[m]);
+}
+
 }  // namespace fm

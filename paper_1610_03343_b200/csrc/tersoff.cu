@@ -203,27 +203,45 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
     }
     const int hhx = __double2hiint(0.5 * Lx), hhy = __double2hiint(0.5 * Ly), hhz = __double2hiint(0.5 * Lz);
 
+    // Every phase below advances all MR slots (or all MR(MR-1)/2 unordered slot pairs) together, one
+    // arithmetic step at a time (fastmath.cuh, *_v): consecutive instructions are independent.
+    constexpr int NP = MR * (MR - 1) / 2;
     T ex[MR], ey[MR], ez[MR], rinv[MR], rr[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
     unsigned mask = 0u, window = 0u;
+    {
+        T d2s[MR], aR[MR], aA[MR];
 #pragma unroll
-    for (int m = 0; m < MR; ++m) {
-        const T tx = (T)min_image_listed(dx[m] - xi, Lx, hhx);
-        const T ty = (T)min_image_listed(dy[m] - yi, Ly, hhy);
-        const T tz = (T)min_image_listed(dz[m] - zi, Lz, hhz);
-        const T d2 = tx * tx + ty * ty + tz * tz;
-        const bool in = m < nn && d2 < p.S2;
-        const T d2s = in ? d2 : T(1);                        // keeps the empty slot's arithmetic finite
-        const T ri = fm::rsqrt(d2s);
-        rr[m] = d2s * ri;
-        ex[m] = tx * ri; ey[m] = ty * ri; ez[m] = tz * ri; rinv[m] = ri;
-        mask |= in ? 1u << m : 0u;
-        window |= (in && rr[m] > p.R) ? 1u << m : 0u;
-        fc[m] = in ? T(1) : T(0);
-        fcp[m] = T(0);
-        const T eR = fm::exp(-p.lambda * rr[m], tb), eA = fm::exp(-p.mu * rr[m], tb);
-        fR[m] = in ? p.A * eR : T(0);
-        fA[m] = in ? p.B * eA : T(0);
-        zeta[m] = T(0);
+        for (int m = 0; m < MR; ++m) {
+            ex[m] = (T)min_image_listed(dx[m] - xi, Lx, hhx);
+            ey[m] = (T)min_image_listed(dy[m] - yi, Ly, hhy);
+            ez[m] = (T)min_image_listed(dz[m] - zi, Lz, hhz);
+        }
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            const T d2 = ex[m] * ex[m] + ey[m] * ey[m] + ez[m] * ez[m];
+            const bool in = m < nn && d2 < p.S2;
+            d2s[m] = in ? d2 : T(1);                         // keeps the empty slot's arithmetic finite
+            mask |= in ? 1u << m : 0u;
+        }
+        fm::rsqrt_v<MR>(d2s, rinv);
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            rr[m] = d2s[m] * rinv[m];
+            ex[m] *= rinv[m]; ey[m] *= rinv[m]; ez[m] *= rinv[m];
+            aR[m] = -p.lambda * rr[m]; aA[m] = -p.mu * rr[m];
+        }
+        fm::exp_v<MR>(aR, fR, tb);
+        fm::exp_v<MR>(aA, fA, tb);
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            const bool in = mask >> m & 1u;
+            window |= (in && rr[m] > p.R) ? 1u << m : 0u;
+            fc[m] = in ? T(1) : T(0);
+            fcp[m] = T(0);
+            fR[m] = in ? p.A * fR[m] : T(0);
+            fA[m] = in ? p.B * fA[m] : T(0);
+            zeta[m] = T(0);
+        }
     }
     if (window) {                                            // f_C window R < r < S (reading A1)
 #pragma unroll
@@ -238,55 +256,88 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
 
     // zeta (Eq. 4), unordered neighbour pairs visited once (g_ijk = g_ikj for one element);
     // g = 1 + (c/d)^2 x^2/(d^2 + x^2), x = h - cos (Eq. 5 without its cancellation)
+    {
+        T x2[NP], den[NP], q[NP];
+        int c = 0;
 #pragma unroll
-    for (int a = 0; a < MR; ++a)
+        for (int a = 0; a < MR; ++a)
 #pragma unroll
-        for (int b = a + 1; b < MR; ++b) {
-            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-            const T xx = p.h - cs;
-            const T x2 = xx * xx;
-            const T g = T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2);
-            zeta[a] += fc[b] * g;
-            zeta[b] += fc[a] * g;
-        }
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T xx = p.h - (ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b]);
+                x2[c] = xx * xx;
+                den[c] = p.d2 + x2[c];
+            }
+        fm::rcp_v<NP>(den, q);
+        c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T g = T(1) + p.c2_over_d2 * x2[c] * q[c];
+                zeta[a] += fc[b] * g;
+                zeta[b] += fc[a] * g;
+            }
+    }
 
     // b_ij, b'_ij (Eq. 3); zeta = 0: b = 1, b' = 0 (reading A8)
     T U = T(0);
     T Px[MR], Py[MR], Pz[MR], hh[MR];
+    {
+        T zt[MR], w1[MR], w2[MR], t[MR], u[MR], bb[MR], rc[MR];
 #pragma unroll
-    for (int a = 0; a < MR; ++a) {
-        const bool pos = zeta[a] > T(0);
-        const T zt = pos ? zeta[a] : T(1);
-        const T t = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);        // (beta zeta)^n
-        const T u = T(1) + t;
-        const T bb = fm::exp(p.minus_half_over_n * fm::log(u, tb), tb); // (1 + t)^(-1/2n)
-        const T b = pos ? bb : T(1);
-        const T bp = pos ? T(-0.5) * bb * t * fm::rcp(zt * u) : T(0);
-        const T bfA = b * fA[a];
-        U += T(0.5) * fc[a] * (fR[a] - bfA);
-        const T D = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
-        hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
-        Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
+        for (int a = 0; a < MR; ++a) { zt[a] = zeta[a] > T(0) ? zeta[a] : T(1); w1[a] = p.beta * zt[a]; }
+        fm::log_v<MR>(w1, w2, tb);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) w2[a] *= p.n;
+        fm::exp_v<MR>(w2, t, tb);                                        // (beta zeta)^n
+#pragma unroll
+        for (int a = 0; a < MR; ++a) { u[a] = T(1) + t[a]; w1[a] = zt[a] * u[a]; }
+        fm::log_v<MR>(u, w2, tb);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) w2[a] *= p.minus_half_over_n;
+        fm::exp_v<MR>(w2, bb, tb);                                       // (1 + t)^(-1/2n)
+        fm::rcp_v<MR>(w1, rc);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) {
+            const T posf = zeta[a] > T(0) ? T(1) : T(0);                 // a factor, not a branch
+            const T b = zeta[a] > T(0) ? bb[a] : T(1);
+            const T bp = T(-0.5) * bb[a] * t[a] * rc[a] * posf;
+            const T bfA = b * fA[a];
+            U += T(0.5) * fc[a] * (fR[a] - bfA);
+            const T D = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
+            hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
+            Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
+        }
     }
 
     // P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g'_ab (e_b - cos e_a)/r_a + h_b fc'_a g_ab e_a ]
+    {
+        T cs[NP], xx[NP], den[NP], q[NP];
+        int c = 0;
 #pragma unroll
-    for (int a = 0; a < MR; ++a)
+        for (int a = 0; a < MR; ++a)
 #pragma unroll
-        for (int b = a + 1; b < MR; ++b) {
-            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-            const T xx = p.h - cs;
-            const T x2 = xx * xx;
-            const T q = fm::rcp(p.d2 + x2);
-            const T g = T(1) + p.c2_over_d2 * x2 * q;
-            const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
-            const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
-            const T ta = tab * rinv[a], tb2 = tab * rinv[b];
-            const T ua = hh[b] * fcp[a] * g - ta * cs;
-            const T ub = hh[a] * fcp[b] * g - tb2 * cs;
-            Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
-            Px[b] += tb2 * ex[a] + ub * ex[b]; Py[b] += tb2 * ey[a] + ub * ey[b]; Pz[b] += tb2 * ez[a] + ub * ez[b];
-        }
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                cs[c] = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+                xx[c] = p.h - cs[c];
+                den[c] = p.d2 + xx[c] * xx[c];
+            }
+        fm::rcp_v<NP>(den, q);
+        c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T g = T(1) + p.c2_over_d2 * xx[c] * xx[c] * q[c];
+                const T gp = T(-2) * p.c2 * xx[c] * q[c] * q[c];         // dg/dcos
+                const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
+                const T ta = tab * rinv[a], tb2 = tab * rinv[b];
+                const T ua = hh[b] * fcp[a] * g - ta * cs[c];
+                const T ub = hh[a] * fcp[b] * g - tb2 * cs[c];
+                Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
+                Px[b] += tb2 * ex[a] + ub * ex[b]; Py[b] += tb2 * ey[a] + ub * ey[b]; Pz[b] += tb2 * ez[a] + ub * ez[b];
+            }
+    }
 
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
