@@ -136,6 +136,21 @@ def traffic_from_profiles(kernel):
         return None
 
 
+def max_over_ranks(values, device, world):
+    """Times of the slowest rank (the contract's max over ranks); identity for one rank."""
+    import torch
+    import torch.distributed as dist
+    tv = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tv, op=dist.ReduceOp.MAX)
+    return [float(v) for v in tv.cpu()]
+
+
+def aggregate_value(n_per_rank, steps, world, ms_max):
+    """Whole-job atom-steps/s of `world` replicas of n_per_rank atoms each, timed by the slowest rank."""
+    return world * n_per_rank * steps / (ms_max * 1e-3)
+
+
 def main_ours(args):
     import torch
     import torch.distributed as dist
@@ -242,10 +257,7 @@ def main_ours(args):
     e2e_s = e2e_call(args.steps)
     md.md_neighbors_status(nl2)
 
-    tv = torch.tensor([ms_total, ms_prof, ms_b2b, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tv, op=dist.ReduceOp.MAX)
-    ms_total, ms_prof, ms_b2b, e2e_ms = [float(v) for v in tv.cpu()]
+    ms_total, ms_prof, ms_b2b, e2e_ms = max_over_ranks([ms_total, ms_prof, ms_b2b, e2e_s * 1e3], dev, world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -258,7 +270,7 @@ def main_ours(args):
     achieved = PAIR_FLOP_PER_ATOM[pot] * n / (pair_ms * 1e-3) / 1e12
     _, long_rows = md.md_neighbors_row_stats(nl)
     kern = "k_sw_pairs_cta" if pot == "sw" else ("k_tersoff_pairs_cta" if long_rows * 256 > n else "k_tersoff_atom")
-    value = world * n * args.steps / (ms_total * 1e-3)
+    value = aggregate_value(n, args.steps, world, ms_total)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,

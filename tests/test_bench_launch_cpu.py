@@ -47,3 +47,35 @@ def test_reference_arm_under_torchrun_two_ranks_prints_once():
     lines = [d for d in json_lines(r.stdout) if d.get("impl") == "reference"]
     assert len(lines) == 1
     assert lines[0]["n_gpus"] == 2 and lines[0]["value"] > 0
+
+
+def _gloo_worker(rank, world, port, out):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    mine = [10.0 + rank, 5.0 - rank, 7.0, 100.0 * (rank + 1)]
+    got = bench.max_over_ranks(mine, "cpu", world)
+    dist.barrier()
+    dist.destroy_process_group()
+    out.put((rank, got))
+
+
+def test_max_over_ranks_and_aggregate_with_gloo_world_size_2():
+    """The replicas' timing reduction (bench.py, N > 1): every rank ends up with the slowest rank's
+    times, and the job value counts all replicas' atoms against that time."""
+    import torch.multiprocessing as mp
+    sys.path.insert(0, ROOT)
+    import bench
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_gloo_worker, args=(r, 2, 29733, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(60)
+        assert p.exitcode == 0
+    assert res[0] == res[1] == [11.0, 5.0, 7.0, 200.0]
+    assert bench.max_over_ranks([3.0, 4.0], "cpu", 1) == [3.0, 4.0]
+    assert bench.aggregate_value(512000, 10, 2, 2.0) == 2 * 512000 * 10 / 2e-3
