@@ -11,7 +11,7 @@ INCLUDE = os.path.join(os.path.dirname(_DIR), "include")
 LIB = os.path.join(_DIR, "libmd_b200.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC", "-shared"]
 
 
 def sources():
@@ -29,7 +29,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + \
+        cmd = [nvcc] + NVCC_FLAGS + \
               (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-I", CSRC, "-o", LIB] + sources()
         subprocess.check_call(cmd)
     return LIB

@@ -56,7 +56,7 @@ compact_in_range(Dense<T, TA, PC>& d, int64_t A0, int na, int64_t n, int K,
         const int q = tid + u * NT;
         const int m = q / TA, t = q - m * TA;
         in[u] = m < KL && m < d.nn[t];
-        jj[u] = in[u] ? NL[(int64_t)m * n + A0 + t] : (int)(A0 + t);
+        jj[u] = in[u] ? NL[(int64_t)m * n + A0 + t] : (int)(A0 + (t < na ? t : 0));   // always a valid atom
     }
 #pragma unroll
     for (int u = 0; u < TPT; ++u) {                          // level 2: coordinates

@@ -248,3 +248,62 @@ def test_total_virial_is_strain_derivative(pot):
             e.append(math.fsum(oo["pe"]))
         dU = (e[0] - e[1]) / (2 * eps)
         assert abs(W[4 * a] + dU) <= 2e-7 * max(1.0, np.abs(W).max())
+
+
+# ---------------------------------------------------------------- P17 elastic constants (three-body magnitude)
+EV_PER_A3_IN_GPA = 160.21766208
+
+
+def strained_lattice_energy(pot, params, a, strain, ncell=2):
+    """Total energy and reference volume of the perfect lattice under a homogeneous diagonal strain
+    (box and positions scaled together; no internal relaxation, which C11 and C12 do not need)."""
+    x, y, z, L = mi.diamond_lattice(ncell, a)
+    s = np.asarray(strain, dtype=float)
+    box = np.array([L, L, L]) * (1.0 + s)
+    rl = (params["S"] if pot == "tersoff" else params["a"] * params["sigma"]) + 0.05
+    NN, NL = oracle.neighbors(x * (1 + s[0]), y * (1 + s[1]), z * (1 + s[2]), box, rl, 40, method="brute")
+    o = oracle.evaluate(pot, params, x * (1 + s[0]), y * (1 + s[1]), z * (1 + s[2]), box, NN, NL, want=("pe",))
+    return math.fsum(o["pe"]), L ** 3
+
+
+def cubic_elastic_constants(pot, params, a, h=1e-3):
+    """C11, C12, B in GPa by central second differences of the energy:
+    E/V = 1/2 C11 sum e_aa^2 + C12 sum_{a<b} e_aa e_bb, so d2E/de_xx^2 = V C11 and, with
+    e_xx = e_yy = e, d2E/de^2 = 2 V (C11 + C12)."""
+    e0, V = strained_lattice_energy(pot, params, a, (0, 0, 0))
+    d2 = lambda s: (strained_lattice_energy(pot, params, a, s)[0] - 2 * e0 +
+                    strained_lattice_energy(pot, params, a, tuple(-c for c in s))[0]) / h ** 2 / V * EV_PER_A3_IN_GPA
+    c11 = d2((h, 0, 0))
+    c12 = 0.5 * d2((h, h, 0)) - c11
+    return c11, c12, (c11 + 2 * c12) / 3
+
+
+def test_sw_elastic_constants_pin_three_body_magnitude():
+    """every other SW pin is blind to the size of V3 (it vanishes on the diamond lattice at any
+    lattice constant; finite-difference pins pass for any lambda, gamma).  C11 - C12 is carried by V3 alone."""
+    g = golden()
+    p = mi.SW_SI
+    a0 = 4 * 2 ** (1 / 6) * p["sigma"] / math.sqrt(3)            # zero-pressure lattice constant (P2)
+    c11, c12, bulk = cubic_elastic_constants("sw", p, a0)
+    for got, key in ((c11, "sw_c11_GPa"), (c12, "sw_c12_GPa"), (bulk, "sw_bulk_GPa")):
+        assert abs(got - g[key][0]) <= g[key][1], (key, got)
+    # the pin has teeth: 5 % in lambda or in gamma fails it
+    for k in ("lam", "gamma"):
+        q = dict(p); q[k] = 0.95 * p[k]
+        bad11, bad12, _ = cubic_elastic_constants("sw", q, a0)
+        assert abs(bad11 - g["sw_c11_GPa"][0]) > 5 * g["sw_c11_GPa"][1], k
+        assert abs(bad12 - g["sw_c12_GPa"][0]) > 3 * g["sw_c12_GPa"][1], k
+
+
+def test_tersoff_elastic_constants_pin_angular_term():
+    """The same pin for g(theta) and b(zeta): Tersoff (1988) fitted Si(C) to improve exactly these."""
+    g = golden()
+    t = mi.TERSOFF_SI_C
+    c11, c12, bulk = cubic_elastic_constants("tersoff", t, g["tersoff_sic_a0_A"][0])
+    for got, key in ((c11, "tersoff_sic_c11_GPa"), (c12, "tersoff_sic_c12_GPa"), (bulk, "tersoff_sic_bulk_GPa")):
+        assert abs(got - g[key][0]) <= g[key][1], (key, got)
+    for k, fac in (("h", 1.05), ("d", 1.05), ("c", 1.05)):
+        q = dict(t); q[k] = fac * t[k]
+        bad11, bad12, _ = cubic_elastic_constants("tersoff", q, g["tersoff_sic_a0_A"][0])
+        assert max(abs(bad11 - g["tersoff_sic_c11_GPa"][0]), abs(bad12 - g["tersoff_sic_c12_GPa"][0])) > \
+            3 * g["tersoff_sic_c11_GPa"][1], k
