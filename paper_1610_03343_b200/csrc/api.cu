@@ -1,6 +1,9 @@
 // api.cu -- the C ABI declared in include/md.h: argument checks, handle life cycle, and the host-side
 // composition of the kernels.  No arithmetic of the method lives here.
+#include <mutex>
 #include <new>
+#include <set>
+#include <utility>
 
 #include "common.cuh"
 
@@ -42,6 +45,20 @@ int check_force_args(md_neighbors* nl, int64_t n, const double* x, const double*
 
 }  // namespace
 
+// Kernels that need more than 48 KB of dynamic shared memory must opt in per device (the attribute belongs
+// to the function on the current device, not to the process).
+int md_allow_dynamic_smem(const void* kernel, int bytes) {
+    static std::mutex mu;
+    static std::set<std::pair<int, const void*>> done;
+    int dev = 0;
+    MD_CUDA_TRY(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count({dev, kernel})) return MD_OK;
+    MD_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    done.insert({dev, kernel});
+    return MD_OK;
+}
+
 // ---- per-kind launch counting and event timing --------------------------------------------------
 ProfScope::ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_) : nl(nl_), s(s_), e1(nullptr), on(false) {
     if (!nl) return;
@@ -61,13 +78,22 @@ ProfScope::ProfScope(md_neighbors* nl_, int kind, int nk, cudaStream_t s_) : nl(
 }
 ProfScope::~ProfScope() { if (on) cudaEventRecord(e1, s); }
 
-int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows) {
+int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows, int wait) {
     if (nl->maxrow_pending) {
-        MD_CUDA_TRY(cudaEventSynchronize(nl->ev_list));
-        nl->maxrow_pending = 0;
+        // the statistics only steer the choice between two kernels that are both correct for any list, so a
+        // force call takes whatever has arrived (no host stall, no idle GPU after a rebuild); only the very
+        // first call, or an explicit md_neighbors_row_stats, waits for the copy
+        cudaError_t q = (wait || !nl->row_stats_valid) ? cudaEventSynchronize(nl->ev_list) : cudaEventQuery(nl->ev_list);
+        if (q == cudaSuccess) {
+            nl->row_stats[0] = nl->h_maxrow[0]; nl->row_stats[1] = nl->h_maxrow[1];
+            nl->row_stats_valid = 1;
+            nl->maxrow_pending = 0;
+        } else if (q != cudaErrorNotReady) {
+            return MD_ERR_CUDA;
+        }
     }
-    *max_row = nl->h_maxrow[0];
-    *long_rows = nl->h_maxrow[1];
+    *max_row = nl->row_stats[0];
+    *long_rows = nl->row_stats[1];
     return MD_OK;
 }
 
@@ -159,7 +185,7 @@ int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than
     if (!nl) return MD_ERR_ARG;
     if (nl->n == 0) return MD_ERR_NO_LIST;
     int a = 0, b = 0;
-    const int rc = md_list_row_stats(nl, &a, &b);
+    const int rc = md_list_row_stats(nl, &a, &b, 1);
     if (rc != MD_OK) return rc;
     if (max_row) *max_row = a;
     if (rows_longer_than_4) *rows_longer_than_4 = b;
@@ -239,6 +265,11 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
     if (n > 0 && (!x || !y || !z || !vx || !vy || !vz || !f)) return MD_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
+    // argument errors have no side effects: everything that can be refused is refused before the first launch
+    for (int a = 0; a < 3; ++a)
+        if ((int)(box[a] / r_list) < 3) return MD_ERR_BOX_TOO_SMALL;
+    const bool first_step_rebuilds = first_step % rebuild_every == 0;
+    if (f_valid && nsteps > 0 && !first_step_rebuilds && nl->n != n) return MD_ERR_NO_LIST;
     if (!f_valid) {
         if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
@@ -293,8 +324,8 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
         MD_CUDA_TRY(cudaMemcpyAsync(host_in[a], d + a * n, bytes, cudaMemcpyDeviceToHost, s));
     if (f) MD_CUDA_TRY(cudaMemcpyAsync(f, d + 6 * n, 3 * bytes, cudaMemcpyDeviceToHost, s));
     if (pe) MD_CUDA_TRY(cudaMemcpyAsync(pe, d + 9 * n, bytes, cudaMemcpyDeviceToHost, s));
-    MD_CUDA_TRY(cudaStreamSynchronize(s));
-    return MD_OK;
+    // this call synchronises anyway, so it reports what the device latched (row or in-range overflow)
+    return md_neighbors_status(nl, nullptr, stream);
 }
 
 int md_probe_fp64_peak(int iters, double* tflops, void* stream) {

@@ -47,9 +47,12 @@ struct md_neighbors {
     int32_t* scan_blocks;   // block sums scratch
     // status
     int* d_status;          // [3]: status bits, max row length seen, number of rows longer than 4
-    // longest row of the current list, mirrored to the host for kernel selection: written by an async
-    // copy at the end of every build / import; the first force call after it waits on the event
-    int* h_maxrow;          // pinned [2]: longest row, number of rows longer than 4
+    // row statistics of the list, mirrored to the host for kernel selection: written by an async copy at
+    // the end of every build / import.  A force call never waits for them (md_list_row_stats(wait = 0)): it
+    // uses the statistics of the last build whose copy has arrived, and waits only if there are none yet.
+    int* h_maxrow;          // pinned [2]: longest row, number of rows longer than 4 (landing zone of the copy)
+    int row_stats[2];       // the last values known to have arrived
+    int row_stats_valid;
     cudaEvent_t ev_list;
     int maxrow_pending;
     // profiling (md_profile_*)
@@ -94,11 +97,20 @@ struct ProfScope {
     ~ProfScope();
 };
 
+// Shared-memory pool of the sorted loop kernels (pair_sort.cuh), in in-range slots per atom of a 128-atom
+// tile.  A warp of the sorted tile takes 32 x (largest M among its atoms) slots, so the caps documented in
+// md.h are: sum over the tile's four warps of that largest M <= 4 x the figure below.
+constexpr int MD_SW_POOL_PER_ATOM = 10;
+constexpr int MD_TERSOFF_POOL_PER_ATOM = 8;
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize, set once per (device, kernel); thread-safe (api.cu)
+int md_allow_dynamic_smem(const void* kernel, int bytes);
+
 // kernels' launchers (defined in the .cu files)
 int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                     const double box[3], double r_list, cudaStream_t s);
 int md_launch_reverse(md_neighbors* nl, cudaStream_t s);
-int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows);   // host copies (may wait for the build)
+int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows, int wait);   // host copies; wait = 1: of the current list
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,

@@ -10,7 +10,7 @@
 //              of a column are contiguous in cell order, so an interior atom scans 9 ranges, not 27.
 //              Rows are kept sorted by index in a shared-memory scratch [K][128] (no local memory) and
 //              stored neighbour-major, NL[m*n+i]
-//   k_reverse  REV[m*n+i] = position of i in row NL[m*n+i]
+//   k_reverse  REV[m*n+i] = position of i in row NL[m*n+i] (binary search on the sorted row)
 #include "common.cuh"
 
 namespace {
@@ -235,11 +235,17 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
     for (int m = 0; m < cnt; ++m) NL[(int64_t)m * n + i] = s_nb[m * SEARCH_BT + tid];
 }
 
-__global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                          uint8_t* __restrict__ REV, int* __restrict__ status) {
+// REV[m*n+i] = position of i in row j = NL[m*n+i].  Rows are sorted by index, so that position is the
+// number of entries of row j smaller than i: a branch-free binary search of fixed depth (the longest row of
+// this list, read from the status word the search kernel just wrote), four searches of a thread interleaved so
+// that their dependent loads overlap.  (Round 1 walked row j entry by entry with an early exit: a chain of
+// up to NN[j] dependent loads per entry, 124 us per build for the 16-18-entry Stillinger-Weber rows.)
+__global__ void __launch_bounds__(128)
+k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+          uint8_t* __restrict__ REV, int* __restrict__ status) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int nn = NN[i];
+    const int nn = min(NN[i], K);
     {   // longest row (also for imported lists): one atomic per warp
         const unsigned act = __activemask();
         const int wmax = __reduce_max_sync(act, nn);
@@ -249,14 +255,39 @@ __global__ void k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, cons
             if (nlong) atomicAdd(&status[2], nlong);
         }
     }
-    for (int m = 0; m < nn; ++m) {
-        const int j = NL[(int64_t)m * n + i];
-        const int nj = NN[j];
-        int mm = -1;
-        for (int q = 0; q < nj; ++q)
-            if (NL[(int64_t)q * n + j] == (int)i) { mm = q; break; }
-        if (mm < 0) { atomicOr(&status[0], MD_DEV_NO_REVERSE); mm = 0; }
-        REV[(int64_t)m * n + i] = (uint8_t)mm;
+    for (int m0 = 0; m0 < nn; m0 += 4) {
+        int j[4], lo[4], hi[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int m = m0 + u < nn ? m0 + u : m0;
+            j[u] = NL[(int64_t)m * n + i];
+            if ((unsigned)j[u] >= (unsigned long long)n) { atomicOr(&status[0], MD_DEV_NO_REVERSE); j[u] = (int)i; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { lo[u] = 0; hi[u] = min(NN[j[u]], K); }
+        // lower bound of i in row j; rows have at most 64 entries: 7 halvings reach lo == hi
+#pragma unroll 1
+        for (int it = 0; it < 7; ++it) {
+            int v[4], mid[4];
+            bool live = false;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                mid[u] = (lo[u] + hi[u]) >> 1;
+                live = live || lo[u] < hi[u];
+                v[u] = lo[u] < hi[u] ? NL[(int64_t)mid[u] * n + j[u]] : 0;
+            }
+            if (!__any_sync(__activemask(), live)) break;
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (lo[u] < hi[u]) { if (v[u] < (int)i) lo[u] = mid[u] + 1; else hi[u] = mid[u]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (m0 + u >= nn) continue;
+            const bool found = lo[u] < min(NN[j[u]], K) && NL[(int64_t)lo[u] * n + j[u]] == (int)i;
+            if (!found) { atomicOr(&status[0], MD_DEV_NO_REVERSE); lo[u] = 0; }
+            REV[(int64_t)(m0 + u) * n + i] = (uint8_t)lo[u];
+        }
     }
 }
 

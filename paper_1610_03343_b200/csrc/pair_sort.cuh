@@ -1,0 +1,194 @@
+// pair_sort.cuh -- front end shared by the loop-structured pair kernels (Tersoff with rows of any length,
+// Stillinger-Weber): per-atom screen of the listed neighbours against the force range, and a CTA-local
+// reassignment of atoms to threads ordered by their number M of in-range neighbours.
+//
+// Why.  The pair arithmetic of one atom costs ~M pair terms + M(M-1) triplet terms.  With one thread per atom
+// in list order a warp runs to the largest M of its 32 lanes: for the Stillinger-Weber list (16-18 listed,
+// 4-12 in range, mean 5.9) that is 2.5x the triplet work actually needed.  After the screen every CTA sorts its
+// BT atoms by M (a counting sort on ballots, deterministic: ties keep list order) and thread `tid` takes the
+// atom of rank `tid`, so the lanes of a warp have (nearly) the same M, the loops over in-range neighbours have
+// warp-uniform trip counts, and no lane idles.  The per-slot data of a thread live in shared-memory columns
+// addressed [slot][lane] inside a region owned by its warp and sized by the warp's largest M, so the CTA's
+// pool is used by what the atoms need (sum over warps of 32 * M_max), not by the worst case of one atom.
+//
+// The screen is the only place where "in range" is decided (one helper, explicit roundings, see in_range_d2):
+// the decision for (i,j) and (j,i) must agree bit for bit, because atom i pushes P_ij into the slot of row j
+// that j's MASK bit says j will read (push layout).
+#pragma once
+#include "common.cuh"
+
+namespace ps {
+
+// d2 of a listed pair, the same roundings wherever MASK is decided (k_tersoff_atom, the generic path, the
+// screen below): dx*dx rounded, then two fused multiply-adds.  x_j - x_i and the minimum-image shift are exact
+// negations of each other for (i,j) and (j,i), so both ends compute the same bits.
+__device__ __forceinline__ double in_range_d2(double dx, double dy, double dz) {
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+}
+__device__ __forceinline__ float in_range_d2(float dx, float dy, float dz) {
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+// Minimum image of a listed pair, coordinates in [0, L).  A pair that needs the +-L shift on some axis has an
+// unwrapped |d_a| > L_a/2, hence an unwrapped d2 > (L_min/2)^2; a pair that does not is (for any list worth
+// the name) far below that.  So the hot path forms d2 from the unwrapped differences and looks at ONE integer
+// compare on its high word (`far`, no FP64-pipe instruction); only when some lane of the warp sees a far pair
+// -- warps at the faces of the box, 1 in 10 at 512 000 atoms -- are the three components tested and shifted
+// and d2 formed again.  d - 0.0 == d, so the result is the same bits whichever path a warp takes, and the
+// shift is an exact negation between (i,j) and (j,i).
+struct MinImage {
+    double Lx, Ly, Lz;
+    int hx, hy, hz;          // high words of L/2
+    int far_hi;              // high word of (min L / 2)^2, rounded down: d2 above it may need a shift
+    static __device__ __forceinline__ double shift(double d, double L, int hi_half) {
+        const int hi = __double2hiint(d);
+        const int sL = __double2hiint(L) | (hi & 0x80000000);            // copysign(L, d), high word
+        const double s = (hi & 0x7fffffff) > hi_half ? __hiloint2double(sL, __double2loint(L)) : 0.0;
+        return d - s;
+    }
+    __device__ __forceinline__ void wrap(double& dx, double& dy, double& dz) const {
+        dx = shift(dx, Lx, hx); dy = shift(dy, Ly, hy); dz = shift(dz, Lz, hz);
+    }
+    // d2 (arithmetic type T) above which a pair may need the shift; T = float rounds d first, hence the margin
+    template <class T> __device__ __forceinline__ bool far(T d2) const {
+        return __double2hiint((double)d2) >= far_hi;
+    }
+};
+
+__device__ __forceinline__ MinImage make_min_image(double lx, double ly, double lz) {
+    MinImage m;
+    m.Lx = lx; m.Ly = ly; m.Lz = lz;
+    m.hx = __double2hiint(0.5 * lx); m.hy = __double2hiint(0.5 * ly); m.hz = __double2hiint(0.5 * lz);
+    const double lm = fmin(lx, fmin(ly, lz));
+    m.far_hi = __double2hiint(0.2499 * lm * lm) - 1;        // a little below (L_min/2)^2: conservative
+    return m;
+}
+
+constexpr int MBINS = 33;        // in-range counts 0..32 (a list row has at most 64 entries; > 32 in range: overflow)
+
+template <int BT>
+struct SortScratch {
+    unsigned long long mask[BT];     // in-range bits over the list row of atom t (tile order)
+    unsigned short perm[BT];         // perm[rank] = t
+    int cnt[BT / 32][MBINS + 3];     // per warp: atoms with M == b; then exclusive offsets (padded: 36 ints)
+    int wmax[BT / 32];               // per warp (after the sort): largest M
+};
+
+// Screen: in-range bit mask of atom i over its list row (thread-per-atom, coalesced row reads, eight
+// neighbours in flight: their list entries first, then their 24 coordinates).  T is the arithmetic type of the
+// force kernel: in FP32 mode r_ij is formed in double, rounded to float, and the float d2 decides (reading
+// A10) -- for both ends.  Indices are 32-bit: n * max_neighbors <= 2e9 is checked at md_neighbors_create.
+template <class T>
+__device__ __forceinline__ unsigned long long
+screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const double* __restrict__ y,
+           const double* __restrict__ z, const MinImage& mi, const int32_t* __restrict__ NL, T range2) {
+    constexpr int U = 8;
+    const double xi = x[i], yi = y[i], zi = z[i];
+    unsigned long long mask = 0ull;
+    for (int m0 = 0; m0 < nn; m0 += U) {
+        int j[U];
+        double dx[U], dy[U], dz[U];
+        T d2[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const unsigned m = m0 + u < nn ? m0 + u : m0;       // a valid row entry for the idle tail
+            j[u] = NL[m * n + i];
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) { dx[u] = x[j[u]] - xi; dy[u] = y[j[u]] - yi; dz[u] = z[j[u]] - zi; }
+        bool far = false;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            d2[u] = in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+            far = far || mi.far(d2[u]);
+        }
+        if (__any_sync(__activemask(), far)) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                mi.wrap(dx[u], dy[u], dz[u]);
+                d2[u] = in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+            }
+        }
+        unsigned bits = 0u;
+#pragma unroll
+        for (int u = 0; u < U; ++u) bits |= d2[u] < range2 ? 1u << u : 0u;
+        const int left = nn - m0;                                // entries of this chunk that exist
+        if (left < U) bits &= (1u << left) - 1u;
+        mask |= (unsigned long long)bits << m0;
+    }
+    return mask;
+}
+
+// Sort the CTA's atoms by M = popc(mask) (ascending, ties in tile order).  On return thread `tid` owns tile
+// atom *t (its mask in *mask), its warp's column region starts at pool slot *base and holds *M_w slots per
+// lane (M_w = largest M in the warp, clamped so that the region fits `pool_slots`; a clamp latches
+// MD_DEV_INRANGE_OVERFLOW and the caller drops the pairs beyond *M_w).  Atoms with t >= na (tile tail) carry
+// mask 0 and sort to the front with M = 0.  Uses four __syncthreads().
+template <int BT>
+__device__ __forceinline__ void
+sort_by_count(SortScratch<BT>& s, unsigned long long my_mask, int pool_slots, int* __restrict__ status,
+              int* t_out, unsigned long long* mask_out, int* base_out, int* Mw_out) {
+    constexpr int NW = BT / 32;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int M = __popcll(my_mask);
+    if (M > MBINS - 1) { atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); M = MBINS - 1; }
+    s.mask[tid] = my_mask;
+    // per-warp histogram on ballots: lane b keeps the count of bin b (bins 32.. fold into lane 0's second word)
+    // (only the bins between the warp's smallest and largest M can be occupied)
+    int mine = 0, mine32 = 0;
+    unsigned same = 0u;
+    const int blo = __reduce_min_sync(0xffffffffu, M), bhi = __reduce_max_sync(0xffffffffu, M);
+#pragma unroll 1
+    for (int b = blo; b <= bhi; ++b) {
+        const unsigned v = __ballot_sync(0xffffffffu, M == b);
+        if (b < 32) { if (lane == b) mine = __popc(v); } else { if (lane == 0) mine32 = __popc(v); }
+        if (M == b) same = v;
+    }
+    s.cnt[wid][lane] = mine;
+    if (lane == 0) s.cnt[wid][32] = mine32;
+    __syncthreads();
+    // warp 0: exclusive offsets, bin-major then warp-major (the order of the sorted sequence)
+    if (wid == 0) {
+        int run = 0;
+#pragma unroll 1
+        for (int b0 = 0; b0 < MBINS; b0 += 32) {
+            const int b = b0 + lane;
+            int c[NW], tot = 0;
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { c[w] = b < MBINS ? s.cnt[w][b] : 0; tot += c[w]; }
+            int inc = tot;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += v;
+            }
+            int off = run + inc - tot;
+            if (b < MBINS) {
+#pragma unroll
+                for (int w = 0; w < NW; ++w) { s.cnt[w][b] = off; off += c[w]; }
+            }
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    __syncthreads();
+    const int rank = s.cnt[wid][M] + __popc(same & ((1u << lane) - 1u));
+    s.perm[rank] = (unsigned short)tid;
+    __syncthreads();
+    const int t = s.perm[tid];
+    const unsigned long long mk = s.mask[t];
+    const int Mt = min(__popcll(mk), MBINS - 1);
+    const int wmax = __reduce_max_sync(0xffffffffu, Mt);
+    if (lane == 0) s.wmax[wid] = wmax;
+    __syncthreads();
+    int base = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) base += w < wid ? 32 * s.wmax[w] : 0;
+    int Mw = wmax;
+    if (base + 32 * Mw > pool_slots) {                       // pool exhausted: keep what fits, flag it
+        if (lane == 0) atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW);
+        Mw = base < pool_slots ? (pool_slots - base) / 32 : 0;
+    }
+    *t_out = t; *mask_out = mk; *base_out = base; *Mw_out = Mw;
+}
+
+}  // namespace ps

@@ -7,9 +7,31 @@
 //        + sum_{k != j} lambda eps s_j s_k [ ds_j delta^2 e_ij + 2 delta (e_ik - cos e_ij)/r_ij ]
 //   s_j = exp(gamma sigma/(r_ij - r_c)), ds_j = -gamma sigma/(r_ij - r_c)^2, delta = cos - cos0.
 // Same push / own-half scheme as tersoff.cu.
+//
+// The three-body sum is separable.  With s_j = exp(gamma sigma/(r_ij - r_c)), c0 = cos0 and the moments
+//   S = sum_j s_j,  S2 = sum_j s_j^2,  v = sum_j s_j e_j,  T = sum_j s_j e_j (x) e_j      (in-range j)
+// one has  sum_{j<k} s_j s_k (e_j.e_k - c0)^2 = 1/2 [ T:T - 2 c0 |v|^2 + c0^2 S^2 - (1 - c0)^2 S2 ],  so
+//   U3_i      = lambda eps / 2 [ T:T - 2 c0 |v|^2 + c0^2 S^2 - (1 - c0)^2 S2 ]
+//   dU3/ds_j  = lambda eps [ e_j.T e_j - 2 c0 v.e_j + c0^2 S - (1 - c0)^2 s_j ]  =: A_j  (= sum_{k!=j} lambda eps s_k delta_jk^2)
+//   dU3/de_j  = 2 lambda eps s_j (T e_j - c0 v) =: g_j   (up to a radial part that the projection removes)
+//   P_ij      = [ V2'/2 + A_j s_j ds_j - (e_j.g_j)/r_ij ] e_j + g_j / r_ij
+// which is term for term the double sum above, evaluated in O(M) per atom instead of O(M^2).  Every term
+// keeps its factor s_j, so a neighbour at the edge of the range still gets full relative accuracy; the
+// cancellation inside A_j and g_j (terms O(S), result O(S delta)) costs ~2 digits of 16.
+//
+// Kernel structure (k_sw_sorted): one thread per atom, loops over the atom's in-range neighbours.  The SW
+// list holds the whole second shell (16-18 entries at the 0.5 A skin) but only 4-12 of them (mean 5.9) are
+// inside r_c, so
+//   screen  every thread tests the listed neighbours of one atom of the CTA's tile (coalesced row reads)
+//           and keeps the in-range bits: that is MASK, stored at once;
+//   sort    the CTA reassigns its atoms to threads in order of M (pair_sort.cuh): warps become M-uniform;
+//   pass 1  per in-range slot: e_ij, r, s_j  -> the thread's shared-memory columns; moments in registers;
+//   pass 2  per slot: two-body terms, A_j, g_j, P_ij pushed to Q[rev(i,j)*n + j]; U_i and the own halves
+//           sum_j P_ij, -1/2 sum_j r_ij (x) P_ij accumulate in registers.
+// Both passes take two slots per iteration (independent chains for the FP64 pipe).
 #include "common.cuh"
 #include "real_math.cuh"
-#include "pair_cta.cuh"
+#include "pair_sort.cuh"
 #include "fastmath.cuh"
 
 namespace {
@@ -17,133 +39,171 @@ namespace {
 template <class T>
 struct SWDev {
     T Aeps, B, sigma, rc, rc2, gs, leps, cos0, p, q;
-    int ip, iq;      // integer exponents if p, q are small non-negative integers, else -1
 };
 
-template <class T> __device__ __forceinline__ T ipow(T a, int e) {
+// (sigma/r)^e: E >= 0 is a compile-time integer exponent, E < 0 means "use pow with the real exponent"
+template <int E, class T> __device__ __forceinline__ T spow(T a, T e) {
+    if (E < 0) return rm::pow(a, e);
     T r = T(1);
-    for (int k = 0; k < e; ++k) r *= a;
+#pragma unroll
+    for (int k = 0; k < E; ++k) r *= a;
     return r;
 }
 
-// "lanes = pairs" kernel.  The SW list holds the whole second shell (16-18 entries at the 0.5 A skin) but
-// only ~6 of them are inside r_c, so a thread-per-atom loop would idle most lanes and spill its per-
-// neighbour arrays.  A CTA of 256 threads owns TA atoms:
-//   stage A  compaction of the in-range pairs into shared memory              (pair_cta.cuh)
-//   stage B  per pair: e_ij, 1/r, V2, V2', s_j = exp(gamma sigma/(r - r_c)), ds_j
-//   stage C  per pair: three-body sums over the other in-range pairs of the same atom, P_ij pushed
-//            to Q[rev(i,m)*n + j]
-//   stage D  per atom: U_i, own halves sum_j P_ij and -1/2 sum_j r_ij (x) P_ij, MASK
-template <class T, int TA, int PC>
+template <class T, int BT, int PCA>
 struct SWSmem {
-    pc::Dense<T, TA, PC> d;
-    T rinv[PC], sj[PC], ds[PC], D[PC], Uh[PC];   // Uh: V2/2, then + the pair's share of the V3 terms
-    T Px[PC], Py[PC], Pz[PC];
+    ps::SortScratch<BT> ss;
+    T ex[PCA * BT], ey[PCA * BT], ez[PCA * BT];   // unit vectors e_ij of the thread's in-range slots
+    T sj[PCA * BT], rr[PCA * BT];                 // s_j and r_ij
     __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
-template <class T, class Rec, int TA, int PC>
-__global__ void __launch_bounds__(pc::NT)
-k_sw_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
-               const double* __restrict__ z, double Lx, double Ly, double Lz,
-               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, SWDev<T> p, const double* __restrict__ gtab,
-               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-               int* __restrict__ status) {
+template <class T, class Rec, int BT, int PCA, int IP, int IQ>
+__global__ void __launch_bounds__(BT)
+k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+            const double* __restrict__ z, double Lx, double Ly, double Lz,
+            const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+            const uint8_t* __restrict__ REV, SWDev<T> p, const double* __restrict__ gtab,
+            Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+            double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+            int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    SWSmem<T, TA, PC>& s = *reinterpret_cast<SWSmem<T, TA, PC>*>(smem_raw);
-    const int tid = threadIdx.x;
-    const int64_t A0 = (int64_t)blockIdx.x * TA;
-    const int na = (int)min((int64_t)TA, n - A0);
-    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after compact_in_range's barriers
-    pc::compact_in_range<T, TA, PC, 32>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.rc2, status);
-    const int np = s.d.np;
+    SWSmem<T, BT, PCA>& s = *reinterpret_cast<SWSmem<T, BT, PCA>*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t A0 = (int64_t)blockIdx.x * BT;
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
-    // stage B
-    for (int k = tid; k < np; k += pc::NT) {
-        const T tx = s.d.ex[k], ty = s.d.ey[k], tz = s.d.ez[k];
-        const T d2 = tx * tx + ty * ty + tz * tz;
-        const T ri = fm::rsqrt(d2);
-        const T rr = d2 * ri;
-        s.d.ex[k] = tx * ri; s.d.ey[k] = ty * ri; s.d.ez[k] = tz * ri; s.rinv[k] = ri;
-        const bool ok = rr < p.rc;                          // never divide by r - r_c = 0 (reading A8)
-        // u = 1/(r - r_c) < 0, clamped at -300: beyond that exp(sigma u) < 1e-270 is zero for every purpose,
-        // and fm::exp wants |argument| < 2e7
-        const T u = ok ? max(fm::rcp(rr - p.rc), T(-300)) : T(-1);
-        // two-body: V2 = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - rc))
-        const T sr = p.sigma * ri;
-        const T sp = p.ip >= 0 ? ipow(sr, p.ip) : rm::pow(sr, p.p);
-        const T sq = p.iq >= 0 ? ipow(sr, p.iq) : rm::pow(sr, p.q);
-        const T ev = ok ? p.Aeps * fm::exp(p.sigma * u, tb) : T(0);
-        const T br = p.B * sp - sq;
-        s.Uh[k] = T(0.5) * ev * br;
-        s.D[k] = T(0.5) * ev * ((p.q * sq - p.p * p.B * sp) * ri - br * p.sigma * u * u);
-        s.sj[k] = ok ? fm::exp(p.gs * u, tb) : T(0);
-        s.ds[k] = -p.gs * u * u;
+    // screen, tile order
+    unsigned long long mask0 = 0ull;
+    if (A0 + tid < n) {
+        const int64_t i0 = A0 + tid;
+        int nn = NN[i0];
+        if (nn > 64) nn = 64;
+        mask0 = ps::screen_row<T>((unsigned)i0, (unsigned)n, nn, x, y, z, mi, NL, p.rc2);
+        MASK[i0] = mask0;
     }
-    __syncthreads();
+    int t, base, Mw;
+    unsigned long long mk;
+    ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
+    const int M = min(__popcll(mk), Mw);
+    if (A0 + t >= n) return;                                 // tile tail (M = 0); no barrier follows
+    const int64_t i = A0 + t;
+    const int col = base + lane;                             // slot k of this thread: col + 32 k
 
-    // stage C: P_a = D_a e_a + sum_{b != a} E [ ds_a delta^2 e_a + 2 delta (e_b - cos e_a)/r_a ],
-    // E = lambda eps s_a s_b, delta = cos - cos0; V3 of a triplet belongs to the central atom (A6)
-    for (int k = tid; k < np; k += pc::NT) {
-        const int tmk = s.d.tm[k];
-        const int t = tmk >> 6, m = tmk & 63;
-        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
-        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
-        const T sa = p.leps * s.sj[k], dsa = s.ds[k], two_ria = T(2) * s.rinv[k];
-        T ce = s.D[k];                                       // coefficient of e_a
-        T sx = T(0), sy = T(0), sz = T(0), u3 = T(0);
-        for (int b = b0; b < b1; ++b) {
-            if (b == k) continue;
-            const T bx = s.d.ex[b], by = s.d.ey[b], bz = s.d.ez[b];
-            const T cs = ax * bx + ay * by + az * bz;
-            const T dl = cs - p.cos0;
-            const T Ed = sa * s.sj[b] * dl;
-            const T Edd = Ed * dl;
-            u3 += Edd;
-            const T ta = Ed * two_ria;
-            ce += Edd * dsa - ta * cs;
-            sx += ta * bx; sy += ta * by; sz += ta * bz;
+    // pass 1: geometry and s_j of every in-range slot; moments S, S2, v, T
+    T S = T(0), S2 = T(0), vx = T(0), vy = T(0), vz = T(0);
+    T Txx = T(0), Txy = T(0), Txz = T(0), Tyy = T(0), Tyz = T(0), Tzz = T(0);
+    {
+        const double xi = x[i], yi = y[i], zi = z[i];
+        unsigned long long run = mk;
+        for (int k0 = 0; k0 < M; k0 += 2) {
+            int j[2];
+            double dx[2], dy[2], dz[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int m = __ffsll((long long)run) - 1;   // run != 0 while k0 + u < M; else m = -1 -> slot 0
+                if (k0 + u < M) run &= run - 1;
+                j[u] = NL[(unsigned)(m < 0 ? 0 : m) * (unsigned)n + (unsigned)i];
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { dx[u] = x[j[u]] - xi; dy[u] = y[j[u]] - yi; dz[u] = z[j[u]] - zi; }
+            T d2s[2];
+            bool far = false;
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+                far = far || mi.far(d2s[u]);
+            }
+            if (__any_sync(__activemask(), far)) {           // warp-uniform: interior warps never shift
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    mi.wrap(dx[u], dy[u], dz[u]);
+                    d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                if (k0 + u >= M) continue;
+                const T tx = (T)dx[u], ty = (T)dy[u], tz = (T)dz[u];
+                const T d2 = d2s[u];
+                const T ri = fm::rsqrt(d2);
+                const T r = d2 * ri;
+                // u = 1/(r - r_c) < 0, clamped at -300: beyond that exp(sigma u) < 1e-270 is zero for every
+                // purpose, and fm::exp wants |argument| < 2e7; never divide by r - r_c = 0 (reading A8)
+                const bool ok = r < p.rc;
+                const T uu = ok ? max(fm::rcp(r - p.rc), T(-300)) : T(-1);
+                const int c = col + 32 * (k0 + u);
+                const T ex = tx * ri, ey = ty * ri, ez = tz * ri;
+                const T sj = ok ? fm::exp(p.gs * uu, tb) : T(0);
+                s.ex[c] = ex; s.ey[c] = ey; s.ez[c] = ez;
+                s.rr[c] = r;
+                s.sj[c] = sj;
+                const T wx = sj * ex, wy = sj * ey, wz = sj * ez;
+                S += sj; S2 += sj * sj;
+                vx += wx; vy += wy; vz += wz;
+                Txx += wx * ex; Txy += wx * ey; Txz += wx * ez;
+                Tyy += wy * ey; Tyz += wy * ez; Tzz += wz * ez;
+            }
         }
-        const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
-        s.Px[k] = px; s.Py[k] = py; s.Pz[k] = pz;
-        s.Uh[k] += T(0.5) * u3;                              // each unordered pair (a,b) is met twice
-        const int64_t i = A0 + t;
-        const int mm = REV[(int64_t)m * n + i];
-        rm::store_rec(&Q[(int64_t)mm * n + s.d.j[k]], px, py, pz);
     }
-    __syncthreads();
 
-    // stage D: per-atom sums
-    for (int t = tid; t < na; t += pc::NT) {
-        const int64_t i = A0 + t;
-        T U = T(0), Fx = T(0), Fy = T(0), Fz = T(0);
-        T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
-        for (int b = s.d.off[t]; b < s.d.off[t + 1]; ++b) {
-            const T px = s.Px[b], py = s.Py[b], pz = s.Pz[b];
-            U += s.Uh[b]; Fx += px; Fy += py; Fz += pz;
+    // pass 2: P_j = [ V2'/2 + A_j s_j ds_j - (e_j.g_j)/r_j ] e_j + g_j/r_j  (header comment)
+    const T c0 = p.cos0, om2 = (T(1) - c0) * (T(1) - c0);
+    const T cvx = c0 * vx, cvy = c0 * vy, cvz = c0 * vz, kS = c0 * c0 * S;
+    T U = T(0.5) * p.leps * (Txx * Txx + Tyy * Tyy + Tzz * Tzz + T(2) * (Txy * Txy + Txz * Txz + Tyz * Tyz)
+                             - T(2) * (cvx * vx + cvy * vy + cvz * vz) + kS * S - om2 * S2);   // V3 of atom i (A6)
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    unsigned long long run = mk;
+    for (int a0 = 0; a0 < M; a0 += 2) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (a0 + u >= M) continue;
+            const int m = __ffsll((long long)run) - 1;
+            run &= run - 1;
+            const int ca = col + 32 * (a0 + u);
+            const T ex = s.ex[ca], ey = s.ey[ca], ez = s.ez[ca], r = s.rr[ca], sj = s.sj[ca];
+            const unsigned mi32 = (unsigned)m * (unsigned)n + (unsigned)i;
+            const int ja = NL[mi32];                         // L1-hot: read by the screen and by pass 1
+            const int mm = REV[mi32];
+            // two-body: V2 = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - rc))
+            const bool ok = r < p.rc;
+            const T ri = fm::rcp(r);
+            const T uu = ok ? max(fm::rcp(r - p.rc), T(-300)) : T(-1);
+            const T sr = p.sigma * ri;
+            const T sp = spow<IP>(sr, p.p), sq = spow<IQ>(sr, p.q);
+            const T ev = ok ? p.Aeps * fm::exp(p.sigma * uu, tb) : T(0);
+            const T br = p.B * sp - sq;
+            const T u2 = uu * uu;
+            const T D = T(0.5) * ev * ((p.q * sq - p.p * p.B * sp) * ri - br * p.sigma * u2);   // V2'/2
+            // three-body through the moments
+            const T wx = Txx * ex + Txy * ey + Txz * ez, wy = Txy * ex + Tyy * ey + Tyz * ez,
+                    wz = Txz * ex + Tyz * ey + Tzz * ez;                                          // T e_j
+            const T q = ex * wx + ey * wy + ez * wz, ve = vx * ex + vy * ey + vz * ez;
+            const T A = p.leps * (q - T(2) * c0 * ve + kS - om2 * sj);
+            const T k2 = T(2) * p.leps * sj;
+            const T gx = k2 * (wx - cvx), gy = k2 * (wy - cvy), gz = k2 * (wz - cvz);             // g_j
+            const T eg = k2 * (q - c0 * ve);                                                      // e_j . g_j
+            const T ce = D - A * sj * p.gs * u2 - eg * ri;                                        // ds_j = -gs u^2
+            const T px = ce * ex + gx * ri, py = ce * ey + gy * ri, pz = ce * ez + gz * ri;
+            rm::store_rec(&Q[(unsigned)mm * (unsigned)n + (unsigned)ja], px, py, pz);
+            U += T(0.5) * ev * br;                           // V2/2
+            Fx += px; Fy += py; Fz += pz;
             if (virial) {
-                const T rr = T(1) / s.rinv[b];
-                const T rx = s.d.ex[b] * rr, ry = s.d.ey[b] * rr, rz = s.d.ez[b] * rr;
+                const T rx = ex * r, ry = ey * r, rz = ez * r;
                 W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
                 W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
                 W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
             }
         }
-        MASK[i] = s.d.mask[t];
-        if (pe) pe[i] = (double)U;
-        if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
-        if (virial) {
-#pragma unroll
-            for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
-        }
     }
-}
-
-inline int small_int(double v) {
-    const int k = (int)v;
-    return ((double)k == v && k >= 0 && k <= 16) ? k : -1;
+    if (pe) pe[i] = (double)U;
+    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+    if (virial) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+    }
 }
 
 template <class T, class Rec>
@@ -154,20 +214,17 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.Aeps = (T)(hp->A * hp->epsilon); p.B = (T)hp->B; p.sigma = (T)hp->sigma;
     p.rc = (T)rc; p.rc2 = (T)(rc * rc); p.gs = (T)(hp->gamma * hp->sigma);
     p.leps = (T)(hp->lambda * hp->epsilon); p.cos0 = (T)hp->cos0; p.p = (T)hp->p; p.q = (T)hp->q;
-    p.ip = small_int(hp->p); p.iq = small_int(hp->q);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
-    constexpr int TA = 40, PC = 16 * TA;                     // ~6 in-range pairs per atom: ~240 per CTA
-    using Sm = SWSmem<T, TA, PC>;
-    auto kern = k_sw_pairs_cta<T, Rec, TA, PC>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        MD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Sm)));
-        attr_set = true;
-    }
-    kern<<<(unsigned)((n + TA - 1) / TA), pc::NT, sizeof(Sm), s>>>(
-        n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
+    constexpr int BT = 128, PCA = MD_SW_POOL_PER_ATOM;
+    using Sm = SWSmem<T, BT, PCA>;
+    // the published exponents (p = 4, q = 0) get compile-time integer powers; anything else goes through pow
+    auto kern = (hp->p == 4.0 && hp->q == 0.0) ? k_sw_sorted<T, Rec, BT, PCA, 4, 0> : k_sw_sorted<T, Rec, BT, PCA, -1, -1>;
+    const int rcs = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
+    if (rcs != MD_OK) return rcs;
+    kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
+        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
         pe, f, virial, nl->d_status);
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;

@@ -12,7 +12,7 @@
 
 #include "common.cuh"
 #include "real_math.cuh"
-#include "pair_cta.cuh"
+#include "pair_sort.cuh"
 #include "fastmath.cuh"
 
 namespace {
@@ -56,7 +56,7 @@ tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const d
         const double dy = md_min_image(y[j] - yi, Ly, hy);
         const double dz = md_min_image(z[j] - zi, Lz, hz);
         const T tx = (T)dx, ty = (T)dy, tz = (T)dz;
-        const T d2 = tx * tx + ty * ty + tz * tz;
+        const T d2 = ps::in_range_d2(tx, ty, tz);
         if (d2 < p.S2) {
             if (M >= TERSOFF_KC) { atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); continue; }
             const T rinv = rm::rsqrt(d2);
@@ -151,77 +151,29 @@ tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const d
     }
 }
 
-// Minimum image of a difference that is known to lie within the list cut-off of 0 or of +-L (a listed
-// pair, coordinates in [0, L)): any threshold between works, so the test is an integer compare on the
-// high word (no FP64-pipe instruction) and the shift one DADD.
-__device__ __forceinline__ double min_image_listed(double d, double L, int hi_half) {
-    const int hi = __double2hiint(d);
-    const int sL = __double2hiint(L) | (hi & 0x80000000);            // copysign(L, d), high word
-    const double shift = (hi & 0x7fffffff) > hi_half ? __hiloint2double(sL, __double2loint(L)) : 0.0;
-    return d - shift;
-}
-
-// Register path: list rows of up to MR entries, every per-neighbour quantity in registers (all array
-// indices are compile-time constants after unrolling).  The arithmetic is one straight basic block over
-// all MR slots, so ptxas interleaves the slots' independent FP64 chains; a slot that is empty or outside
-// the force range carries f_C = f_C' = f_R = f_A = 0 and drops out of every sum.  The only branch is the
-// (rare) cut-off window R < r < S.
-template <class T, class Rec, int MR, int BT, int MAXREG>
-__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
-k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
-               const double* __restrict__ z, double Lx, double Ly, double Lz,
-               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
-               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-               int* __restrict__ status) {
-    // Loads first, in two dependent levels only: {NN, NL, REV, math tables} -> {x[j]}.  The list slots are
-    // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
-    // index and masked out below), and the table staging's barrier comes after the loads are in flight.
-    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
-    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t i = i0 < n ? i0 : n - 1;
-    const int nn = NN[i];
-    int jd[MR], rv[MR];
-#pragma unroll
-    for (int m = 0; m < MR; ++m) {
-        const int mk = m < K ? m : 0;
-        const int jr = NL[(int64_t)mk * n + i];
-        jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
-        rv[m] = (int)REV[(int64_t)mk * n + i];
-    }
-    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
-    const double xi = x[i], yi = y[i], zi = z[i];
-    double dx[MR], dy[MR], dz[MR];
-#pragma unroll
-    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
-    __syncthreads();
-    if (i0 >= n) return;
-    if (nn > MR) {
-        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, virial, status);
-        return;
-    }
-    const int hhx = __double2hiint(0.5 * Lx), hhy = __double2hiint(0.5 * Ly), hhz = __double2hiint(0.5 * Lz);
-
-    // Every phase below advances all MR slots (or all MR(MR-1)/2 unordered slot pairs) together, one
-    // arithmetic step at a time (fastmath.cuh, *_v): consecutive instructions are independent.
+// Register body: up to MR neighbour slots, every per-neighbour quantity in registers (all array indices are
+// compile-time constants after unrolling).  The arithmetic is one straight basic block over all MR slots, so
+// ptxas interleaves the slots' independent FP64 chains; a slot that is empty or outside the force range
+// (bit clear in `mask`) carries f_C = f_C' = f_R = f_A = 0 and drops out of every sum.  The only branch is
+// the (rare) cut-off window R < r < S.  Inputs: raw r_ij of the slots (minimum image applied), the partner
+// index jd and the reverse slot rv of each.  Every phase advances all MR slots (or all MR(MR-1)/2 unordered
+// slot pairs) together, one arithmetic step at a time (fastmath.cuh, *_v): consecutive instructions are
+// independent.
+template <class T, class Rec, int MR>
+__device__ __forceinline__ void
+tersoff_reg_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], unsigned mask,
+                 const int (&jd)[MR], const int (&rv)[MR], const TersoffDev<T>& p, const fm::Tab& tb,
+                 Rec* __restrict__ Q, double* __restrict__ pe, double* __restrict__ f,
+                 double* __restrict__ virial) {
     constexpr int NP = MR * (MR - 1) / 2;
-    T ex[MR], ey[MR], ez[MR], rinv[MR], rr[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
-    unsigned mask = 0u, window = 0u;
+    T rinv[MR], rr[MR], fc[MR], fcp[MR], fR[MR], fA[MR], zeta[MR];
+    unsigned window = 0u;
     {
         T d2s[MR], aR[MR], aA[MR];
 #pragma unroll
         for (int m = 0; m < MR; ++m) {
-            ex[m] = (T)min_image_listed(dx[m] - xi, Lx, hhx);
-            ey[m] = (T)min_image_listed(dy[m] - yi, Ly, hhy);
-            ez[m] = (T)min_image_listed(dz[m] - zi, Lz, hhz);
-        }
-#pragma unroll
-        for (int m = 0; m < MR; ++m) {
-            const T d2 = ex[m] * ex[m] + ey[m] * ey[m] + ez[m] * ez[m];
-            const bool in = m < nn && d2 < p.S2;
-            d2s[m] = in ? d2 : T(1);                         // keeps the empty slot's arithmetic finite
-            mask |= in ? 1u << m : 0u;
+            const T d2 = ps::in_range_d2(ex[m], ey[m], ez[m]);
+            d2s[m] = (mask >> m & 1u) ? d2 : T(1);           // keeps the empty slot's arithmetic finite
         }
         fm::rsqrt_v<MR>(d2s, rinv);
 #pragma unroll
@@ -353,7 +305,6 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
                 W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
             }
         }
-    MASK[i] = (unsigned long long)mask;
     if (pe) pe[i] = (double)U;
     if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
     if (virial) {
@@ -362,139 +313,286 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
     }
 }
 
+
+// Thread-per-atom kernel for crystal rows (at most MR listed entries): slot m is list position m.
+template <class T, class Rec, int MR, int BT, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
+k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
+               const double* __restrict__ z, double Lx, double Ly, double Lz,
+               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
+               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+               int* __restrict__ status) {
+    // Loads first, in two dependent levels only: {NN, NL, REV, math tables} -> {x[j]}.  The list slots are
+    // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
+    // index and masked out below), and the table staging's barrier comes after the loads are in flight.
+    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = i0 < n ? i0 : n - 1;
+    const int nn = NN[i];
+    int jd[MR], rv[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) {
+        const int mk = m < K ? m : 0;
+        const int jr = NL[(int64_t)mk * n + i];
+        jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
+        rv[m] = (int)REV[(int64_t)mk * n + i];
+    }
+    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    const double xi = x[i], yi = y[i], zi = z[i];
+    double dx[MR], dy[MR], dz[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
+    __syncthreads();
+    if (i0 >= n) return;
+    if (nn > MR) {
+        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, virial, status);
+        return;
+    }
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
+    T ex[MR], ey[MR], ez[MR];
+    unsigned mask = 0u;
+    {
+        double qx[MR], qy[MR], qz[MR];
+        T d2[MR];
+        bool far = false;
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            qx[m] = dx[m] - xi; qy[m] = dy[m] - yi; qz[m] = dz[m] - zi;
+            d2[m] = ps::in_range_d2((T)qx[m], (T)qy[m], (T)qz[m]);       // the one in-range decision (pair_sort.cuh)
+            far = far || mi.far(d2[m]);
+        }
+        if (__any_sync(__activemask(), far)) {               // warp-uniform: interior warps never shift
+#pragma unroll
+            for (int m = 0; m < MR; ++m) {
+                mi.wrap(qx[m], qy[m], qz[m]);
+                d2[m] = ps::in_range_d2((T)qx[m], (T)qy[m], (T)qz[m]);
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            ex[m] = (T)qx[m]; ey[m] = (T)qy[m]; ez[m] = (T)qz[m];
+            mask |= (m < nn && d2[m] < p.S2) ? 1u << m : 0u;
+        }
+    }
+    MASK[i] = (unsigned long long)mask;
+    tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
+}
+
 // ---------------------------------------------------------------------------------------------------
-// "lanes = pairs" kernel (default).  CTA of 256 threads owns TA atoms; one thread per in-range pair.
-//   stage A  compaction of the in-range pairs into shared memory            (pair_cta.cuh)
-//   stage B  per pair: e_ij, 1/r, f_C, f_C', f_R, f_A
-//   stage C  per pair: zeta_ij over the other pairs of the same atom, b_ij, b'_ij, U_ij/2, D, h
-//   stage D  per pair: P_ij (T5), pushed to Q[rev(i,m)*n + j]
-//   stage E  per atom: U_i, own halves sum_j P_ij and -1/2 sum_j r_ij (x) P_ij, MASK
-template <class T, int TA, int PC>
-struct TersoffSmem {
-    pc::Dense<T, TA, PC> d;
-    T rinv[PC], fc[PC], fcp[PC], fRD[PC], fAu[PC], hh[PC];   // fRD: f_R then D; fAu: f_A then U_ij/2
-    T Px[PC], Py[PC], Pz[PC];
+// Loop kernel for list rows of any length (config 5: 4-9 listed, 3-6 in range; rows longer than 4 are what
+// the register kernel cannot hold).  One thread per atom; the CTA first screens its atoms and reassigns them
+// to threads in order of their in-range count M (pair_sort.cuh), so the loops below have warp-uniform trip
+// counts.  Per-slot data live in the thread's shared-memory columns.
+//   pass 1  per slot: e_ij, 1/r, f_C, f_C', f_R, f_A
+//   pass 2  per slot a: zeta_ia over the other slots, b, b', U_ia/2; D_a and h_a replace f_R, f_A
+//   pass 3  per slot a: P_ia (T5), pushed to Q[rev(i,a)*n + j_a]; own halves in registers
+// Ordered pairs (a,b) and (b,a) are both visited: nothing here relies on g_ijk = g_ikj.
+// Warps whose atoms all have at most RMR in-range neighbours leave the loops for the register body above.
+template <class T, int BT, int PCA>
+struct TersoffSortSmem {
+    ps::SortScratch<BT> ss;
+    T ex[PCA * BT], ey[PCA * BT], ez[PCA * BT], rinv[PCA * BT];
+    T fc[PCA * BT], fcp[PCA * BT], fRD[PCA * BT], fAh[PCA * BT];   // fRD: f_R then D; fAh: f_A then h
+    int jj[PCA * BT];
     __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
-template <class T, class Rec, int TA, int PC>
-__global__ void __launch_bounds__(pc::NT)
-k_tersoff_pairs_cta(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
-                    const double* __restrict__ z, double Lx, double Ly, double Lz,
-                    const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                    const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
-                    Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-                    double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-                    int* __restrict__ status) {
+template <class T, class Rec, int BT, int PCA, int RMR, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
+k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                 const double* __restrict__ z, double Lx, double Ly, double Lz,
+                 const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                 const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
+                 Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+                 double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+                 int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    TersoffSmem<T, TA, PC>& s = *reinterpret_cast<TersoffSmem<T, TA, PC>*>(smem_raw);
-    const int tid = threadIdx.x;
-    const int64_t A0 = (int64_t)blockIdx.x * TA;
-    const int na = (int)min((int64_t)TA, n - A0);
-    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after compact_in_range's barriers
-    pc::compact_in_range<T, TA, PC, 16>(s.d, A0, na, n, K, x, y, z, Lx, Ly, Lz, NN, NL, p.S2, status);
-    const int np = s.d.np;
+    TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t A0 = (int64_t)blockIdx.x * BT;
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
-    // stage B
-    for (int k = tid; k < np; k += pc::NT) {
-        const T tx = s.d.ex[k], ty = s.d.ey[k], tz = s.d.ez[k];
-        const T d2 = tx * tx + ty * ty + tz * tz;
-        const T ri = fm::rsqrt(d2);
-        const T rr = d2 * ri;
-        s.d.ex[k] = tx * ri; s.d.ey[k] = ty * ri; s.d.ez[k] = tz * ri; s.rinv[k] = ri;
-        T c = T(1), cp = T(0);
-        if (rr > p.R) {                                      // f_C window R < r < S (reading A1)
-            T sn, cs;
-            fm::sincos_0_pi((rr - p.R) * p.w, &sn, &cs);
-            c = T(0.5) + T(0.5) * cs;
-            cp = T(-0.5) * p.w * sn;
-        }
-        s.fc[k] = c; s.fcp[k] = cp;
-        s.fRD[k] = p.A * fm::exp(-p.lambda * rr, tb);
-        s.fAu[k] = p.B * fm::exp(-p.mu * rr, tb);
+    unsigned long long mask0 = 0ull;
+    if (A0 + tid < n) {
+        const int64_t i0 = A0 + tid;
+        int nn = NN[i0];
+        if (nn > 64) nn = 64;
+        mask0 = ps::screen_row<T>((unsigned)i0, (unsigned)n, nn, x, y, z, mi, NL, p.S2);
+        MASK[i0] = mask0;
     }
-    __syncthreads();
+    int t, base, Mw;
+    unsigned long long mk;
+    ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
+    const int M = min(__popcll(mk), Mw);
+    if (A0 + t >= n) return;                                 // tile tail (M = 0); no barrier follows
+    const int64_t i = A0 + t;
+    const int col = base + lane;                             // slot k of this thread: col + 32 k
 
-    // stage C: zeta_ij = sum_{k != j} f_C(r_ik) g_ijk (Eq. 4); g in the cancellation-free form
-    for (int k = tid; k < np; k += pc::NT) {
-        const int t = s.d.tm[k] >> 6;
-        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
-        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
+    if (Mw <= RMR) {
+        // every atom of this warp has at most RMR in-range neighbours (after the sort: most warps of a hot
+        // crystal): compact them into register slots and run the straight-line register body
+        int jd[RMR], rv[RMR];
+        unsigned long long run = mk;
+#pragma unroll
+        for (int k = 0; k < RMR; ++k) {
+            const int m = run ? __ffsll((long long)run) - 1 : 0;
+            jd[k] = run ? NL[(int64_t)m * n + i] : (int)i;   // an empty slot points at the atom itself
+            rv[k] = (int)REV[(int64_t)m * n + i];
+            run &= run - 1;
+        }
+        const double xi = x[i], yi = y[i], zi = z[i];
+        double qx[RMR], qy[RMR], qz[RMR];
+        bool far = false;
+#pragma unroll
+        for (int k = 0; k < RMR; ++k) {
+            qx[k] = x[jd[k]] - xi; qy[k] = y[jd[k]] - yi; qz[k] = z[jd[k]] - zi;
+            far = far || mi.far(ps::in_range_d2((T)qx[k], (T)qy[k], (T)qz[k]));
+        }
+        if (__any_sync(__activemask(), far)) {
+#pragma unroll
+            for (int k = 0; k < RMR; ++k) mi.wrap(qx[k], qy[k], qz[k]);
+        }
+        T ex[RMR], ey[RMR], ez[RMR];
+#pragma unroll
+        for (int k = 0; k < RMR; ++k) { ex[k] = (T)qx[k]; ey[k] = (T)qy[k]; ez[k] = (T)qz[k]; }
+        tersoff_reg_body<T, Rec, RMR>(i, n, ex, ey, ez, (1u << M) - 1u, jd, rv, p, tb, Q, pe, f, virial);
+        return;
+    }
+
+    // pass 1
+    {
+        const double xi = x[i], yi = y[i], zi = z[i];
+        unsigned long long run = mk;
+        for (int k0 = 0; k0 < M; k0 += 2) {
+            int j[2];
+            double dx[2], dy[2], dz[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int m = __ffsll((long long)run) - 1;
+                if (k0 + u < M) run &= run - 1;
+                j[u] = NL[(unsigned)(m < 0 ? 0 : m) * (unsigned)n + (unsigned)i];
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { dx[u] = x[j[u]] - xi; dy[u] = y[j[u]] - yi; dz[u] = z[j[u]] - zi; }
+            T d2s[2];
+            bool far = false;
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+                far = far || mi.far(d2s[u]);
+            }
+            if (__any_sync(__activemask(), far)) {           // warp-uniform: interior warps never shift
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    mi.wrap(dx[u], dy[u], dz[u]);
+                    d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                if (k0 + u >= M) continue;
+                const T tx = (T)dx[u], ty = (T)dy[u], tz = (T)dz[u];
+                const T d2 = d2s[u];
+                const T ri = fm::rsqrt(d2);
+                const T r = d2 * ri;
+                T c = T(1), cp = T(0);
+                if (r > p.R) {                               // f_C window R < r < S (reading A1)
+                    T sn, cs;
+                    fm::sincos_0_pi((r - p.R) * p.w, &sn, &cs);
+                    c = T(0.5) + T(0.5) * cs;
+                    cp = T(-0.5) * p.w * sn;
+                }
+                const int q = col + 32 * (k0 + u);
+                s.ex[q] = tx * ri; s.ey[q] = ty * ri; s.ez[q] = tz * ri; s.rinv[q] = ri;
+                s.fc[q] = c; s.fcp[q] = cp;
+                s.fRD[q] = p.A * fm::exp(-p.lambda * r, tb);
+                s.fAh[q] = p.B * fm::exp(-p.mu * r, tb);
+                s.jj[q] = j[u];
+            }
+        }
+    }
+
+    // pass 2: zeta_a = sum_{b != a} f_C(r_b) g_ab (Eq. 4), g in the cancellation-free form; b, b' (Eq. 3)
+    T U = T(0);
+    // (this pass reads only e and f_C of the other slots, so D and h can replace f_R and f_A of slot a at once)
+    for (int a = 0; a < M; ++a) {
+        const int ca = col + 32 * a;
+        const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
         T zt = T(0);
-        for (int b = b0; b < b1; ++b) {
-            if (b == k) continue;
-            const T cs = ax * s.d.ex[b] + ay * s.d.ey[b] + az * s.d.ez[b];
+        auto zterm = [&](int b) {
+            const int cb = col + 32 * b;
+            const T cs = ax * s.ex[cb] + ay * s.ey[cb] + az * s.ez[cb];
             const T xx = p.h - cs;
             const T x2 = xx * xx;
-            zt += s.fc[b] * (T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2));
-        }
+            zt += s.fc[cb] * (T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2));
+        };
+#pragma unroll 2
+        for (int b = 0; b < a; ++b) zterm(b);
+#pragma unroll 2
+        for (int b = a + 1; b < M; ++b) zterm(b);
         T bo = T(1), bp = T(0);
         if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
             const T tt = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);               // (beta zeta)^n
             bo = fm::exp(p.minus_half_over_n * fm::log(T(1) + tt, tb), tb);         // Eq. (3)
             bp = T(-0.5) * bo * tt * fm::rcp(zt * (T(1) + tt));
         }
-        const T c = s.fc[k], cp = s.fcp[k], fR = s.fRD[k], fA = s.fAu[k];
+        const T c = s.fc[ca], cp = s.fcp[ca], fR = s.fRD[ca], fA = s.fAh[ca];
         const T bfA = bo * fA;
-        s.fAu[k] = T(0.5) * c * (fR - bfA);                                            // U_ij / 2
-        s.fRD[k] = T(0.5) * (cp * (fR - bfA) + c * (p.mu * bfA - p.lambda * fR));      // D
-        s.hh[k] = T(-0.5) * c * fA * bp;                                               // h
+        U += T(0.5) * c * (fR - bfA);                                                  // U_ia / 2
+        s.fRD[ca] = T(0.5) * (cp * (fR - bfA) + c * (p.mu * bfA - p.lambda * fR));     // D
+        s.fAh[ca] = T(-0.5) * c * fA * bp;                                             // h
     }
-    __syncthreads();
 
-    // stage D: P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g' (e_b - cos e_a)/r_a + h_b fc'_a g e_a ]
-    for (int k = tid; k < np; k += pc::NT) {
-        const int tmk = s.d.tm[k];
-        const int t = tmk >> 6, m = tmk & 63;
-        const int b0 = s.d.off[t], b1 = s.d.off[t + 1];
-        const T ax = s.d.ex[k], ay = s.d.ey[k], az = s.d.ez[k];
-        const T ha = s.hh[k], ca = s.fc[k], cpa = s.fcp[k], ria = s.rinv[k];
-        T ce = s.fRD[k];                                     // coefficient of e_a
+    // pass 3: P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g' (e_b - cos e_a)/r_a + h_b fc'_a g e_a ]
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    unsigned long long run = mk;
+    for (int a = 0; a < M; ++a) {
+        const int m = __ffsll((long long)run) - 1;
+        run &= run - 1;
+        const int ca = col + 32 * a;
+        const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
+        const T ha = s.fAh[ca], fca = s.fc[ca], cpa = s.fcp[ca], ria = s.rinv[ca];
+        const int ja = s.jj[ca];
+        const int mm = REV[(int64_t)m * n + i];
+        T ce = s.fRD[ca];                                    // coefficient of e_a
         T sx = T(0), sy = T(0), sz = T(0);                   // sum of ta * e_b
-        for (int b = b0; b < b1; ++b) {
-            if (b == k) continue;
-            const T bx = s.d.ex[b], by = s.d.ey[b], bz = s.d.ez[b];
+        auto fterm = [&](int b) {
+            const int cb = col + 32 * b;
+            const T bx = s.ex[cb], by = s.ey[cb], bz = s.ez[cb];
             const T cs = ax * bx + ay * by + az * bz;
             const T xx = p.h - cs;
             const T x2 = xx * xx;
             const T q = fm::rcp(p.d2 + x2);
-            const T hb = s.hh[b];
+            const T hb = s.fAh[cb];
             const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
-            const T ta = (ha * s.fc[b] + hb * ca) * gp * ria;
+            const T ta = (ha * s.fc[cb] + hb * fca) * gp * ria;
             ce += hb * cpa * (T(1) + p.c2_over_d2 * x2 * q) - ta * cs;
             sx += ta * bx; sy += ta * by; sz += ta * bz;
-        }
+        };
+#pragma unroll 2
+        for (int b = 0; b < a; ++b) fterm(b);
+#pragma unroll 2
+        for (int b = a + 1; b < M; ++b) fterm(b);
         const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
-        s.Px[k] = px; s.Py[k] = py; s.Pz[k] = pz;
-        const int64_t i = A0 + t;
-        const int mm = REV[(int64_t)m * n + i];
-        rm::store_rec(&Q[(int64_t)mm * n + s.d.j[k]], px, py, pz);
-    }
-    __syncthreads();
-
-    // stage E: per-atom sums
-    for (int t = tid; t < na; t += pc::NT) {
-        const int64_t i = A0 + t;
-        T U = T(0), Fx = T(0), Fy = T(0), Fz = T(0);
-        T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
-        for (int b = s.d.off[t]; b < s.d.off[t + 1]; ++b) {
-            const T px = s.Px[b], py = s.Py[b], pz = s.Pz[b];
-            U += s.fAu[b]; Fx += px; Fy += py; Fz += pz;
-            if (virial) {
-                const T rr = T(1) / s.rinv[b];
-                const T rx = s.d.ex[b] * rr, ry = s.d.ey[b] * rr, rz = s.d.ez[b] * rr;
-                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
-                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
-                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
-            }
-        }
-        MASK[i] = s.d.mask[t];
-        if (pe) pe[i] = (double)U;
-        if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+        rm::store_rec(&Q[(int64_t)mm * n + ja], px, py, pz);
+        Fx += px; Fy += py; Fz += pz;
         if (virial) {
-#pragma unroll
-            for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+            const T r = fm::rcp(ria);
+            const T rx = ax * r, ry = ay * r, rz = az * r;
+            W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+            W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+            W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
         }
+    }
+    if (pe) pe[i] = (double)U;
+    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+    if (virial) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
     }
 }
 
@@ -518,21 +616,18 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     // Kernel selection by the row lengths of the list (known on the host once per build): the register
     // kernel handles rows of up to 4 entries (the crystal) in its fast path and longer ones through a slow
     // per-thread fallback, so it is used while fewer than 1 row in 256 is longer; otherwise the
-    // lanes = pairs CTA kernel, whose cost does not depend on the row length.
+    // sorted loop kernel (k_tersoff_sorted), which handles rows of any length.
     int max_row = 0, long_rows = 0;
-    const int rcs = md_list_row_stats(nl, &max_row, &long_rows);
+    const int rcs = md_list_row_stats(nl, &max_row, &long_rows, 0);
     if (rcs != MD_OK) return rcs;
     if ((int64_t)long_rows * 256 > n) {
-        constexpr int TA = 64, PC = 8 * TA;
-        using Sm = TersoffSmem<T, TA, PC>;
-        auto kern = k_tersoff_pairs_cta<T, Rec, TA, PC>;
-        static bool attr_set = false;
-        if (!attr_set) {
-            MD_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Sm)));
-            attr_set = true;
-        }
-        kern<<<(unsigned)((n + TA - 1) / TA), pc::NT, sizeof(Sm), s>>>(
-            n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
+        constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
+        using Sm = TersoffSortSmem<T, BT, PCA>;
+        auto kern = k_tersoff_sorted<T, Rec, BT, PCA, 4, 168>;
+        const int rca = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
+        if (rca != MD_OK) return rca;
+        kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
+            n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
             pe, f, virial, nl->d_status);
         MD_CUDA_TRY(cudaGetLastError());
         return MD_OK;

@@ -35,8 +35,7 @@ class GpuSystem:
         torch.cuda.synchronize()
         NN = NN.cpu().numpy()
         NL = NL.cpu().numpy().T.copy()                  # -> atom-major [n][K] like the oracle
-        for i in range(self.n):
-            NL[i, NN[i]:] = -1
+        NL[np.arange(self.K)[None, :] >= NN[:, None]] = -1
         return NN, NL
 
     def import_list(self, NN, NL):
@@ -86,9 +85,9 @@ def assert_close_energy(got, ref, rel=1e-12):
 
 
 def assert_close_fp32(name, got, ref, rel=1e-4):
-    """DESIGN.md A10: ||d||_2 <= rel ||ref||_2 and per-atom |d_i| <= 10 rel * RMS_k |ref_k|."""
+    """DESIGN.md A10 (SURVEY.md reading A10): ||d||_2 <= rel ||ref||_2 and per-atom |d_i| <= rel * RMS_k |ref_k|."""
     d = got - ref
     assert np.linalg.norm(d) <= rel * np.linalg.norm(ref), (name, np.linalg.norm(d) / np.linalg.norm(ref))
     per_atom = np.sqrt((d ** 2).sum(axis=0))
     rms = np.sqrt((ref ** 2).sum(axis=0).mean())
-    assert per_atom.max() <= rel * rms * 10, (name, per_atom.max() / rms)
+    assert per_atom.max() <= rel * rms, (name, per_atom.max() / rms)

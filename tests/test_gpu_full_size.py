@@ -59,6 +59,7 @@ def test_config5_fp32_mode_against_fp64_oracle():
     ref = oracle.evaluate("tersoff", c["params"], c["x"], c["y"], c["z"], c["box"], rNN, rNL,
                           v=(c["vx"], c["vy"], c["vz"]))
     assert abs(out["pe"].sum() - ref["pe"].sum()) <= 1e-4 * abs(ref["pe"].sum())
+    assert_close_energy(out["pe"], ref["pe"], rel=1e-4)              # per atom (reading A10)
     assert_close_fp32("f", out["f"], ref["f"])
     assert_close_fp32("virial", out["virial"], ref["virial"])
     assert_close_fp32("heat", out["heat"], ref["heat"])
