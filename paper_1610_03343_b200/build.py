@@ -29,7 +29,8 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + \
+        extra = os.environ.get("MD_NVCC_EXTRA", "").split()       # e.g. -DMD_SW_MAXREG=168 for an A/B build
+        cmd = [nvcc] + NVCC_FLAGS + extra + \
               (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-I", CSRC, "-o", LIB] + sources()
         subprocess.check_call(cmd)
     return LIB

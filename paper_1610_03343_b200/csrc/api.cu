@@ -209,7 +209,7 @@ int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const in
     MD_CUDA_TRY(cudaMemsetAsync(nl->d_status + 1, 0, 2 * sizeof(int), s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NN, NN, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, s));
     MD_CUDA_TRY(cudaMemcpyAsync(nl->NL, NL, sizeof(int32_t) * n * nl->K, cudaMemcpyDeviceToDevice, s));
-    return md_launch_reverse(nl, s);
+    return md_launch_reverse(nl, s, 1);
 }
 
 int md_build_neighbors(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,

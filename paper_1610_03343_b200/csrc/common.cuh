@@ -37,6 +37,8 @@ struct md_neighbors {
     // per-pair records, pushed layout: Q[m*n + i] = P_{j i}, j = NL[m][i]
     void* Q;                // K*n*32 bytes
     unsigned long long* MASK;  // [n] bit m set <=> slot m is inside the force range
+    int q_dense;            // layout of the records the last pair kernel wrote: 1 = slot counts in-range entries
+                            // (sorted kernels, MASK known beforehand), 0 = slot is the list position
     // cell structures
     int64_t cell_cap;
     int32_t* cell_count;    // [ncell+1] -> exclusive scan in place = cell_start
@@ -100,7 +102,7 @@ struct ProfScope {
 // Shared-memory pool of the sorted loop kernels (pair_sort.cuh), in in-range slots per atom of a 128-atom
 // tile.  A warp of the sorted tile takes 32 x (largest M among its atoms) slots, so the caps documented in
 // md.h are: sum over the tile's four warps of that largest M <= 4 x the figure below.
-constexpr int MD_SW_POOL_PER_ATOM = 10;
+constexpr int MD_SW_POOL_PER_ATOM = 12;
 constexpr int MD_TERSOFF_POOL_PER_ATOM = 8;
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize, set once per (device, kernel); thread-safe (api.cu)
@@ -109,7 +111,7 @@ int md_allow_dynamic_smem(const void* kernel, int bytes);
 // kernels' launchers (defined in the .cu files)
 int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                     const double box[3], double r_list, cudaStream_t s);
-int md_launch_reverse(md_neighbors* nl, cudaStream_t s);
+int md_launch_reverse(md_neighbors* nl, cudaStream_t s, int check);   // check = 1: imported list (verify symmetry)
 int md_list_row_stats(md_neighbors* nl, int* max_row, int* long_rows, int wait);   // host copies; wait = 1: of the current list
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],

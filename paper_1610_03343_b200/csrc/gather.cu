@@ -16,8 +16,8 @@ __global__ void __launch_bounds__(256)
 k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
          const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NL, const Rec* __restrict__ Q,
-         const unsigned long long* __restrict__ MASK, double* __restrict__ f, double* __restrict__ virial,
-         double* __restrict__ heat) {
+         const unsigned long long* __restrict__ MASK, int dense, double* __restrict__ f,
+         double* __restrict__ virial, double* __restrict__ heat) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     unsigned long long mask = MASK[i];
@@ -29,11 +29,13 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
     T Jx = T(0), Jy = T(0), Jz = T(0);
+    int slot = 0;
     while (mask) {
         const int m = __ffsll((long long)mask) - 1;
         mask &= mask - 1;
         T px, py, pz;
-        rm::load_rec(&Q[(int64_t)m * n + i], &px, &py, &pz);
+        rm::load_rec(&Q[(int64_t)(dense ? slot : m) * n + i], &px, &py, &pz);
+        ++slot;
         Fx += px; Fy += py; Fz += pz;
         if (geom) {
             const int j = NL[(int64_t)m * n + i];
@@ -68,7 +70,7 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
 // k_kick_drift (integrate.cu), so the trajectory is bit-identical to the unfused composition.
 template <class T, class Rec, int MODE>
 __global__ void __launch_bounds__(256)
-k_gather_vv(int64_t n, const Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+k_gather_vv(int64_t n, const Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK, int dense,
             double* __restrict__ f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
             double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
             double hk, double dt, double Lx, double Ly, double Lz) {
@@ -80,12 +82,21 @@ k_gather_vv(int64_t n, const Rec* __restrict__ Q, const unsigned long long* __re
     double px = 0, py = 0, pz = 0;
     if (MODE == 2) { px = x[i]; py = y[i]; pz = z[i]; }
     T Fx = T(0), Fy = T(0), Fz = T(0);
-    while (mask) {
-        const int m = __ffsll((long long)mask) - 1;
-        mask &= mask - 1;
-        T qx, qy, qz;
-        rm::load_rec(&Q[(int64_t)m * n + i], &qx, &qy, &qz);
-        Fx += qx; Fy += qy; Fz += qz;
+    if (dense) {                                             // popc(mask) consecutive slots
+        const int cnt = __popcll(mask);
+        for (int sl = 0; sl < cnt; ++sl) {
+            T qx, qy, qz;
+            rm::load_rec(&Q[(int64_t)sl * n + i], &qx, &qy, &qz);
+            Fx += qx; Fy += qy; Fz += qz;
+        }
+    } else {
+        while (mask) {
+            const int m = __ffsll((long long)mask) - 1;
+            mask &= mask - 1;
+            T qx, qy, qz;
+            rm::load_rec(&Q[(int64_t)m * n + i], &qx, &qy, &qz);
+            Fx += qx; Fy += qy; Fz += qz;
+        }
     }
     const double fx = ox - (double)Fx, fy = oy - (double)Fy, fz = oz - (double)Fz;
     ux = __fma_rn(hk, fx, ux); uy = __fma_rn(hk, fy, uy); uz = __fma_rn(hk, fz, uz);     // kick of this step
@@ -110,7 +121,7 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
 #define MD_GATHER_VV(TT, RR, MODE)                                                                        \
-    k_gather_vv<TT, RR, MODE><<<gb, 256, 0, s>>>(n, (const RR*)nl->Q, nl->MASK, f, vv->x, vv->y, vv->z,   \
+    k_gather_vv<TT, RR, MODE><<<gb, 256, 0, s>>>(n, (const RR*)nl->Q, nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z,   \
                                                  vv->vx, vv->vy, vv->vz, vv->hk, vv->dt, box[0], box[1], box[2])
         if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }
         else { if (vv->mode == 2) MD_GATHER_VV(double, PairRec64, 2); else MD_GATHER_VV(double, PairRec64, 1); }
@@ -120,10 +131,10 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     }
     if (precision == MD_FP32)
         k_gather<float, float4><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
-                                                   (const float4*)nl->Q, nl->MASK, f, virial, heat);
+                                                   (const float4*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat);
     else
         k_gather<double, PairRec64><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
-                                                       (const PairRec64*)nl->Q, nl->MASK, f, virial, heat);
+                                                       (const PairRec64*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat);
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
 }

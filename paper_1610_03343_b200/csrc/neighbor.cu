@@ -240,6 +240,9 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
 // this list, read from the status word the search kernel just wrote), four searches of a thread interleaved so
 // that their dependent loads overlap.  (Round 1 walked row j entry by entry with an early exit: a chain of
 // up to NN[j] dependent loads per entry, 124 us per build for the 16-18-entry Stillinger-Weber rows.)
+// CHECK = true (imported lists): every entry is range-checked and the hit verified, a miss latches
+// MD_DEV_NO_REVERSE.  Lists built by k_search are symmetric by construction (the predicate is) and skip that.
+template <bool CHECK>
 __global__ void __launch_bounds__(128)
 k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
           uint8_t* __restrict__ REV, int* __restrict__ status) {
@@ -261,7 +264,7 @@ k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __res
         for (int u = 0; u < 4; ++u) {
             const int m = m0 + u < nn ? m0 + u : m0;
             j[u] = NL[(int64_t)m * n + i];
-            if ((unsigned)j[u] >= (unsigned long long)n) { atomicOr(&status[0], MD_DEV_NO_REVERSE); j[u] = (int)i; }
+            if (CHECK && (unsigned)j[u] >= (unsigned long long)n) { atomicOr(&status[0], MD_DEV_NO_REVERSE); j[u] = (int)i; }
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) { lo[u] = 0; hi[u] = min(NN[j[u]], K); }
@@ -284,8 +287,10 @@ k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __res
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             if (m0 + u >= nn) continue;
-            const bool found = lo[u] < min(NN[j[u]], K) && NL[(int64_t)lo[u] * n + j[u]] == (int)i;
-            if (!found) { atomicOr(&status[0], MD_DEV_NO_REVERSE); lo[u] = 0; }
+            if (CHECK) {
+                const bool found = lo[u] < min(NN[j[u]], K) && NL[(int64_t)lo[u] * n + j[u]] == (int)i;
+                if (!found) { atomicOr(&status[0], MD_DEV_NO_REVERSE); lo[u] = 0; }
+            }
             REV[(int64_t)(m0 + u) * n + i] = (uint8_t)lo[u];
         }
     }
@@ -293,11 +298,12 @@ k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __res
 
 }  // namespace
 
-int md_launch_reverse(md_neighbors* nl, cudaStream_t s) {
+int md_launch_reverse(md_neighbors* nl, cudaStream_t s, int check) {
     const int64_t n = nl->n;
     if (n == 0) return MD_OK;
     ProfScope prof(nl, MD_KIND_BUILD, 1, s);
-    k_reverse<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
+    if (check) k_reverse<true><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
+    else k_reverse<false><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
     MD_CUDA_TRY(cudaGetLastError());
     MD_CUDA_TRY(cudaMemcpyAsync(nl->h_maxrow, nl->d_status + 1, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     MD_CUDA_TRY(cudaEventRecord(nl->ev_list, s));
@@ -356,5 +362,5 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
         n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K, rc2_lo, rc2_hi, nl->NN, nl->NL, nl->d_status);
     }
     MD_CUDA_TRY(cudaGetLastError());
-    return md_launch_reverse(nl, s);
+    return md_launch_reverse(nl, s, 0);
 }

@@ -74,15 +74,14 @@ struct SortScratch {
     int wmax[BT / 32];               // per warp (after the sort): largest M
 };
 
-// Screen: in-range bit mask of atom i over its list row (thread-per-atom, coalesced row reads, eight
-// neighbours in flight: their list entries first, then their 24 coordinates).  T is the arithmetic type of the
+// Screen: in-range bit mask of atom i over its list row (thread-per-atom, coalesced row reads, U
+// neighbours in flight: their list entries first, then their 3 U coordinates).  T is the arithmetic type of the
 // force kernel: in FP32 mode r_ij is formed in double, rounded to float, and the float d2 decides (reading
 // A10) -- for both ends.  Indices are 32-bit: n * max_neighbors <= 2e9 is checked at md_neighbors_create.
-template <class T>
+template <class T, int U>
 __device__ __forceinline__ unsigned long long
 screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const double* __restrict__ y,
            const double* __restrict__ z, const MinImage& mi, const int32_t* __restrict__ NL, T range2) {
-    constexpr int U = 8;
     const double xi = x[i], yi = y[i], zi = z[i];
     unsigned long long mask = 0ull;
     for (int m0 = 0; m0 < nn; m0 += U) {
@@ -117,6 +116,52 @@ screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const d
         mask |= (unsigned long long)bits << m0;
     }
     return mask;
+}
+
+// The screen as a kernel of its own: MASK[i] for every atom.  It is bound by the latency of the two dependent
+// loads (list entry -> coordinates), so it runs with small CTAs and few registers at full occupancy instead
+// of inside the pair kernel (whose shared-memory pool holds it to 12-16 warps per SM), and it makes every
+// MASK known before any pair record is written, which is what the dense record layout needs (dense_slot).
+template <class T>
+__global__ void __launch_bounds__(256, 4)
+k_screen(unsigned n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+         double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+         T range2, unsigned long long* __restrict__ MASK) {
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const MinImage mi = make_min_image(Lx, Ly, Lz);
+    int nn = NN[i];
+    if (nn > 64) nn = 64;
+    MASK[i] = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, range2);
+}
+
+// Dense record layout: the record of pair (i -> j) goes to the slot of row j that counts the in-range entries
+// of row j before i's position rev, so the gather of j reads popc(MASK_j) consecutive slots (coalesced over
+// atoms) instead of the in-range ones scattered over a 16-18-entry row.
+__device__ __forceinline__ unsigned dense_slot(unsigned long long mask_j, int rev) {
+    return (unsigned)__popcll(mask_j & ((1ull << rev) - 1ull));
+}
+
+// A load the compiler may not sink to its first use (prefetch of the next chunk's data into registers).
+__device__ __forceinline__ double ld_early(const double* p) {
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int ld_early(const int32_t* p) {
+    int v;
+    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int ld_early(const uint8_t* p) {
+    int v;
+    asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ unsigned long long ld_early(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.global.nc.u64 %0, [%1];" : "=l"(v) : "l"(p));
+    return v;
 }
 
 // Sort the CTA's atoms by M = popc(mask) (ascending, ties in tile order).  On return thread `tid` owns tile

@@ -58,13 +58,16 @@ struct SWSmem {
     __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
-template <class T, class Rec, int BT, int PCA, int IP, int IQ>
-__global__ void __launch_bounds__(BT)
+#ifndef MD_SW_MAXREG
+#define MD_SW_MAXREG 168     // 3 CTAs of 128 threads per SM; measured: 128 registers (4 CTAs) spills and is 30 % slower
+#endif
+template <class T, class Rec, int BT, int PCA, int IP, int IQ, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
 k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
             const double* __restrict__ z, double Lx, double Ly, double Lz,
             const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
             const uint8_t* __restrict__ REV, SWDev<T> p, const double* __restrict__ gtab,
-            Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+            Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
             double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
             int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -74,15 +77,8 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
-    // screen, tile order
-    unsigned long long mask0 = 0ull;
-    if (A0 + tid < n) {
-        const int64_t i0 = A0 + tid;
-        int nn = NN[i0];
-        if (nn > 64) nn = 64;
-        mask0 = ps::screen_row<T>((unsigned)i0, (unsigned)n, nn, x, y, z, mi, NL, p.rc2);
-        MASK[i0] = mask0;
-    }
+    // in-range masks of the tile (k_screen wrote them), tile order
+    const unsigned long long mask0 = A0 + tid < n ? MASK[A0 + tid] : 0ull;
     int t, base, Mw;
     unsigned long long mk;
     ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
@@ -96,18 +92,39 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
     T Txx = T(0), Txy = T(0), Txz = T(0), Tyy = T(0), Tyz = T(0), Tzz = T(0);
     {
         const double xi = x[i], yi = y[i], zi = z[i];
+        const unsigned n32 = (unsigned)n, i32 = (unsigned)i;
         unsigned long long run = mk;
-        for (int k0 = 0; k0 < M; k0 += 2) {
-            int j[2];
-            double dx[2], dy[2], dz[2];
+        // Two-deep software pipeline over chunks of two slots: while chunk c is worked on, the coordinates of
+        // chunk c+1 and the list entries of chunk c+2 are in flight (the list entry -> coordinate chain is two
+        // dependent loads; ld_early pins the requests where they are written).
+        double cx[2], cy[2], cz[2], nx[2], ny[2], nz[2];
+        int jq[2];
+        auto req_idx = [&](int k0, int (&j)[2]) {
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
                 const int m = __ffsll((long long)run) - 1;   // run != 0 while k0 + u < M; else m = -1 -> slot 0
                 if (k0 + u < M) run &= run - 1;
-                j[u] = NL[(unsigned)(m < 0 ? 0 : m) * (unsigned)n + (unsigned)i];
+                j[u] = ps::ld_early(&NL[(unsigned)(m < 0 ? 0 : m) * n32 + i32]);
             }
+        };
+        auto req_xyz = [&](const int (&j)[2], double (&fx)[2], double (&fy)[2], double (&fz)[2]) {
 #pragma unroll
-            for (int u = 0; u < 2; ++u) { dx[u] = x[j[u]] - xi; dy[u] = y[j[u]] - yi; dz[u] = z[j[u]] - zi; }
+            for (int u = 0; u < 2; ++u) {
+                fx[u] = ps::ld_early(&x[j[u]]); fy[u] = ps::ld_early(&y[j[u]]); fz[u] = ps::ld_early(&z[j[u]]);
+            }
+        };
+        {
+            int j0[2];
+            req_idx(0, j0);
+            req_idx(2, jq);
+            req_xyz(j0, cx, cy, cz);
+        }
+        for (int k0 = 0; k0 < M; k0 += 2) {
+            if (k0 + 2 < M) req_xyz(jq, nx, ny, nz);
+            if (k0 + 4 < M) req_idx(k0 + 4, jq);
+            double dx[2], dy[2], dz[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { dx[u] = cx[u] - xi; dy[u] = cy[u] - yi; dz[u] = cz[u] - zi; }
             T d2s[2];
             bool far = false;
 #pragma unroll
@@ -122,29 +139,40 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
                     d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
                 }
             }
+            // Both slots advance together, one arithmetic step at a time, with no branch between them (a slot
+            // past the atom's last one computes on d2 = 1 and contributes s_j = 0), so that consecutive FP64
+            // instructions are independent.
+            bool val[2], ok[2];
+            T ri[2], r[2], um[2], uu[2], arg[2], sj[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { val[u] = k0 + u < M; d2s[u] = val[u] ? d2s[u] : T(1); }
+            fm::rsqrt_v<2>(d2s, ri);
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                if (k0 + u >= M) continue;
-                const T tx = (T)dx[u], ty = (T)dy[u], tz = (T)dz[u];
-                const T d2 = d2s[u];
-                const T ri = fm::rsqrt(d2);
-                const T r = d2 * ri;
-                // u = 1/(r - r_c) < 0, clamped at -300: beyond that exp(sigma u) < 1e-270 is zero for every
-                // purpose, and fm::exp wants |argument| < 2e7; never divide by r - r_c = 0 (reading A8)
-                const bool ok = r < p.rc;
-                const T uu = ok ? max(fm::rcp(r - p.rc), T(-300)) : T(-1);
+                r[u] = d2s[u] * ri[u];
+                ok[u] = val[u] && r[u] < p.rc;               // never divide by r - r_c = 0 (reading A8)
+                um[u] = ok[u] ? r[u] - p.rc : T(-1);
+            }
+            fm::rcp_v<2>(um, uu);
+            // u = 1/(r - r_c) < 0, clamped at -300: beyond that exp(sigma u) < 1e-270 is zero for every purpose,
+            // and fm::exp wants |argument| < 2e7
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { uu[u] = max(uu[u], T(-300)); arg[u] = p.gs * uu[u]; }
+            fm::exp_v<2>(arg, sj, tb);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                sj[u] = ok[u] ? sj[u] : T(0);
+                const T ex = (T)dx[u] * ri[u], ey = (T)dy[u] * ri[u], ez = (T)dz[u] * ri[u];
                 const int c = col + 32 * (k0 + u);
-                const T ex = tx * ri, ey = ty * ri, ez = tz * ri;
-                const T sj = ok ? fm::exp(p.gs * uu, tb) : T(0);
-                s.ex[c] = ex; s.ey[c] = ey; s.ez[c] = ez;
-                s.rr[c] = r;
-                s.sj[c] = sj;
-                const T wx = sj * ex, wy = sj * ey, wz = sj * ez;
-                S += sj; S2 += sj * sj;
+                if (val[u]) { s.ex[c] = ex; s.ey[c] = ey; s.ez[c] = ez; s.rr[c] = r[u]; s.sj[c] = sj[u]; }
+                const T wx = sj[u] * ex, wy = sj[u] * ey, wz = sj[u] * ez;
+                S += sj[u]; S2 += sj[u] * sj[u];
                 vx += wx; vy += wy; vz += wz;
                 Txx += wx * ex; Txy += wx * ey; Txz += wx * ez;
                 Tyy += wy * ey; Tyz += wy * ez; Tzz += wz * ez;
             }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { cx[u] = nx[u]; cy[u] = ny[u]; cz[u] = nz[u]; }
         }
     }
 
@@ -155,48 +183,85 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
                              - T(2) * (cvx * vx + cvy * vy + cvz * vz) + kS * S - om2 * S2);   // V3 of atom i (A6)
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    // the record slot of pair (i -> j) needs NL -> MASK[j] (two dependent loads): same two-deep pipeline
+    const unsigned n32 = (unsigned)n, i32 = (unsigned)i;
     unsigned long long run = mk;
-    for (int a0 = 0; a0 < M; a0 += 2) {
+    int qj[2], qr[2], cj[2], cr[2], nj[2], nr[2];            // requested / current / next: partner index, rev
+    unsigned long long cm[2], nm[2];                         // MASK of the partner
+    auto req_jr = [&](int k0, int (&j)[2], int (&r)[2]) {
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
-            if (a0 + u >= M) continue;
             const int m = __ffsll((long long)run) - 1;
-            run &= run - 1;
-            const int ca = col + 32 * (a0 + u);
-            const T ex = s.ex[ca], ey = s.ey[ca], ez = s.ez[ca], r = s.rr[ca], sj = s.sj[ca];
-            const unsigned mi32 = (unsigned)m * (unsigned)n + (unsigned)i;
-            const int ja = NL[mi32];                         // L1-hot: read by the screen and by pass 1
-            const int mm = REV[mi32];
+            if (k0 + u < M) run &= run - 1;
+            const unsigned q = (unsigned)(m < 0 ? 0 : m) * n32 + i32;
+            j[u] = ps::ld_early(&NL[q]);
+            r[u] = ps::ld_early(&REV[q]);
+        }
+    };
+    auto req_mask = [&](const int (&j)[2], unsigned long long (&mj)[2]) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) mj[u] = ps::ld_early(&MASK[j[u]]);
+    };
+    req_jr(0, cj, cr);
+    req_jr(2, qj, qr);
+    req_mask(cj, cm);
+    for (int a0 = 0; a0 < M; a0 += 2) {
+        if (a0 + 2 < M) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { nj[u] = qj[u]; nr[u] = qr[u]; }
+            req_mask(nj, nm);
+        }
+        if (a0 + 4 < M) req_jr(a0 + 4, qj, qr);
+        // both slots together, stage by stage, branch-free (a slot past the last one re-reads slot M-1 and is
+        // masked out of the store and the sums)
+        bool val[2], ok[2];
+        T ex[2], ey[2], ez[2], r[2], sj[2], um[2], ri[2], uu[2], arg[2], ev[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            val[u] = a0 + u < M;
+            const int ca = col + 32 * min(a0 + u, M - 1);
+            ex[u] = s.ex[ca]; ey[u] = s.ey[ca]; ez[u] = s.ez[ca]; r[u] = s.rr[ca]; sj[u] = s.sj[ca];
+            ok[u] = r[u] < p.rc;
+            um[u] = ok[u] ? r[u] - p.rc : T(-1);
+        }
+        fm::rcp_v<2>(r, ri);
+        fm::rcp_v<2>(um, uu);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) { uu[u] = max(uu[u], T(-300)); arg[u] = p.sigma * uu[u]; }
+        fm::exp_v<2>(arg, ev, tb);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
             // two-body: V2 = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - rc))
-            const bool ok = r < p.rc;
-            const T ri = fm::rcp(r);
-            const T uu = ok ? max(fm::rcp(r - p.rc), T(-300)) : T(-1);
-            const T sr = p.sigma * ri;
+            const T evu = ok[u] ? p.Aeps * ev[u] : T(0);
+            const T sr = p.sigma * ri[u];
             const T sp = spow<IP>(sr, p.p), sq = spow<IQ>(sr, p.q);
-            const T ev = ok ? p.Aeps * fm::exp(p.sigma * uu, tb) : T(0);
             const T br = p.B * sp - sq;
-            const T u2 = uu * uu;
-            const T D = T(0.5) * ev * ((p.q * sq - p.p * p.B * sp) * ri - br * p.sigma * u2);   // V2'/2
+            const T u2 = uu[u] * uu[u];
+            const T D = T(0.5) * evu * ((p.q * sq - p.p * p.B * sp) * ri[u] - br * p.sigma * u2);   // V2'/2
             // three-body through the moments
-            const T wx = Txx * ex + Txy * ey + Txz * ez, wy = Txy * ex + Tyy * ey + Tyz * ez,
-                    wz = Txz * ex + Tyz * ey + Tzz * ez;                                          // T e_j
-            const T q = ex * wx + ey * wy + ez * wz, ve = vx * ex + vy * ey + vz * ez;
-            const T A = p.leps * (q - T(2) * c0 * ve + kS - om2 * sj);
-            const T k2 = T(2) * p.leps * sj;
-            const T gx = k2 * (wx - cvx), gy = k2 * (wy - cvy), gz = k2 * (wz - cvz);             // g_j
-            const T eg = k2 * (q - c0 * ve);                                                      // e_j . g_j
-            const T ce = D - A * sj * p.gs * u2 - eg * ri;                                        // ds_j = -gs u^2
-            const T px = ce * ex + gx * ri, py = ce * ey + gy * ri, pz = ce * ez + gz * ri;
-            rm::store_rec(&Q[(unsigned)mm * (unsigned)n + (unsigned)ja], px, py, pz);
-            U += T(0.5) * ev * br;                           // V2/2
+            const T wx = Txx * ex[u] + Txy * ey[u] + Txz * ez[u], wy = Txy * ex[u] + Tyy * ey[u] + Tyz * ez[u],
+                    wz = Txz * ex[u] + Tyz * ey[u] + Tzz * ez[u];                                   // T e_j
+            const T q = ex[u] * wx + ey[u] * wy + ez[u] * wz, ve = vx * ex[u] + vy * ey[u] + vz * ez[u];
+            const T A = p.leps * (q - T(2) * c0 * ve + kS - om2 * sj[u]);
+            const T k2 = T(2) * p.leps * sj[u];
+            const T gx = k2 * (wx - cvx), gy = k2 * (wy - cvy), gz = k2 * (wz - cvz);               // g_j
+            const T eg = k2 * (q - c0 * ve);                                                        // e_j . g_j
+            const T ce = D - A * sj[u] * p.gs * u2 - eg * ri[u];                                    // ds_j = -gs u^2
+            const T keep = val[u] ? T(1) : T(0);
+            const T px = keep * (ce * ex[u] + gx * ri[u]), py = keep * (ce * ey[u] + gy * ri[u]),
+                    pz = keep * (ce * ez[u] + gz * ri[u]);
+            if (val[u]) rm::store_rec(&Q[ps::dense_slot(cm[u], cr[u]) * n32 + (unsigned)cj[u]], px, py, pz);
+            U += keep * T(0.5) * evu * br;                   // V2/2
             Fx += px; Fy += py; Fz += pz;
             if (virial) {
-                const T rx = ex * r, ry = ey * r, rz = ez * r;
+                const T rx = ex[u] * r[u], ry = ey[u] * r[u], rz = ez[u] * r[u];
                 W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
                 W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
                 W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
             }
         }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) { cj[u] = nj[u]; cr[u] = nr[u]; cm[u] = nm[u]; }
     }
     if (pe) pe[i] = (double)U;
     if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
@@ -216,11 +281,15 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.leps = (T)(hp->lambda * hp->epsilon); p.cos0 = (T)hp->cos0; p.p = (T)hp->p; p.q = (T)hp->q;
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
-    ProfScope prof(nl, MD_KIND_PAIR, 1, s);
+    ProfScope prof(nl, MD_KIND_PAIR, 2, s);
+    ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2], nl->NN,
+                                                                 nl->NL, p.rc2, nl->MASK);
+    nl->q_dense = 1;
     constexpr int BT = 128, PCA = MD_SW_POOL_PER_ATOM;
     using Sm = SWSmem<T, BT, PCA>;
     // the published exponents (p = 4, q = 0) get compile-time integer powers; anything else goes through pow
-    auto kern = (hp->p == 4.0 && hp->q == 0.0) ? k_sw_sorted<T, Rec, BT, PCA, 4, 0> : k_sw_sorted<T, Rec, BT, PCA, -1, -1>;
+    auto kern = (hp->p == 4.0 && hp->q == 0.0) ? k_sw_sorted<T, Rec, BT, PCA, 4, 0, MD_SW_MAXREG>
+                                                   : k_sw_sorted<T, Rec, BT, PCA, -1, -1, MD_SW_MAXREG>;
     const int rcs = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
     if (rcs != MD_OK) return rcs;
     kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(

@@ -415,14 +415,8 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
-    unsigned long long mask0 = 0ull;
-    if (A0 + tid < n) {
-        const int64_t i0 = A0 + tid;
-        int nn = NN[i0];
-        if (nn > 64) nn = 64;
-        mask0 = ps::screen_row<T>((unsigned)i0, (unsigned)n, nn, x, y, z, mi, NL, p.S2);
-        MASK[i0] = mask0;
-    }
+    // in-range masks of the tile (k_screen wrote them), tile order
+    const unsigned long long mask0 = A0 + tid < n ? MASK[A0 + tid] : 0ull;
     int t, base, Mw;
     unsigned long long mk;
     ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
@@ -443,6 +437,8 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
             rv[k] = (int)REV[(int64_t)m * n + i];
             run &= run - 1;
         }
+#pragma unroll
+        for (int k = 0; k < RMR; ++k) rv[k] = (int)ps::dense_slot(MASK[jd[k]], rv[k]);   // dense record layout
         const double xi = x[i], yi = y[i], zi = z[i];
         double qx[RMR], qy[RMR], qz[RMR];
         bool far = false;
@@ -557,7 +553,7 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
         const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
         const T ha = s.fAh[ca], fca = s.fc[ca], cpa = s.fcp[ca], ria = s.rinv[ca];
         const int ja = s.jj[ca];
-        const int mm = REV[(int64_t)m * n + i];
+        const unsigned slot = ps::dense_slot(MASK[ja], (int)REV[(int64_t)m * n + i]);   // dense record layout
         T ce = s.fRD[ca];                                    // coefficient of e_a
         T sx = T(0), sy = T(0), sz = T(0);                   // sum of ta * e_b
         auto fterm = [&](int b) {
@@ -578,7 +574,7 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
 #pragma unroll 2
         for (int b = a + 1; b < M; ++b) fterm(b);
         const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
-        rm::store_rec(&Q[(int64_t)mm * n + ja], px, py, pz);
+        rm::store_rec(&Q[slot * (unsigned)n + (unsigned)ja], px, py, pz);
         Fx += px; Fy += py; Fz += pz;
         if (virial) {
             const T r = fm::rcp(ria);
@@ -621,6 +617,10 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     const int rcs = md_list_row_stats(nl, &max_row, &long_rows, 0);
     if (rcs != MD_OK) return rcs;
     if ((int64_t)long_rows * 256 > n) {
+        nl->launches[MD_KIND_PAIR] += 1;
+        ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2],
+                                                                     nl->NN, nl->NL, p.S2, nl->MASK);
+        nl->q_dense = 1;
         constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
         using Sm = TersoffSortSmem<T, BT, PCA>;
         auto kern = k_tersoff_sorted<T, Rec, BT, PCA, 4, 168>;
@@ -632,6 +632,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         MD_CUDA_TRY(cudaGetLastError());
         return MD_OK;
     }
+    nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
     MD_TERSOFF_LAUNCH(4, 128, 168);
 #undef MD_TERSOFF_LAUNCH
     MD_CUDA_TRY(cudaGetLastError());
