@@ -1,12 +1,16 @@
 #!/usr/bin/env python
 """bench.py -- atom-steps/s of the FP64 Tersoff/SW force + NVE hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference] [--only-headline]
 
 A "step" is one velocity-Verlet NVE step of the whole hot path (kick+drift, neighbour rebuild every
 10th step, pair kernel, gather, kick) on BASELINE.json config I (default 1 = configs[1]: Tersoff,
-512 000 atoms).  Prints ONE JSON line.  N > 1 runs independent replicas
-(the path is single-GPU by north_star: "replicas only"), one process per GPU under torchrun.
+512 000 atoms).  Prints ONE JSON line: the headline config in the contract's
+keys, and under `configs` a bounded run of every other BASELINE config (3, 4, 5, 5 in FP32 as NVE runs;
+config 1 and the 512 000-atom crystal as full-output evaluations in atom-evals/s), each with its exact
+pair / triplet counts, the pair phase's fraction of the measured FP64 peak and the whole step's fraction of
+the measured HBM bandwidth.  `--config 0` alone prints config 1's evaluation line.  N > 1 runs independent
+replicas (the path is single-GPU by north_star: "replicas only"), one process per GPU under torchrun.
 """
 from __future__ import annotations
 
@@ -27,10 +31,33 @@ import md_inputs as mi  # noqa: E402
 
 METRIC = "atom-steps/s (FP64 Tersoff/SW force+integrate)"
 UNIT = "atom-steps/s"
-# Algorithmic work of the dominant kernel (pair kernel): flop-equivalents per atom
-# with add = mul = 1, fma = 2, div = 16, sqrt = 20, exp = 35, log = 50.
-PAIR_FLOP_PER_ATOM = {"tersoff": 1370.0 + 340.0 + 300.0, "sw": 2300.0}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk x 1.965 GHz = 37.2
+
+
+def pair_flop_equiv(pot, listed, in_range, triplets):
+    """Algorithmic work of one pair phase in flop-equivalents (SURVEY.md section 8(d):
+    add = mul = 1, fma = 2, div = 16, sqrt = 20, exp = 35, log = 50), from EXACT integer counts of listed
+    directed pairs, in-range directed pairs and ordered in-range triplets (md_pair_counts).
+    Tersoff: 342 per in-range pair + (28 zeta pass + 25 force pass) per ordered triplet (M = 4: 2004 per atom).
+    SW: 20 per listed pair (screen) + 178 per in-range pair + 30 per ordered triplet -- the definition's
+    count; the kernel evaluates the triplet sum through moments and executes fewer."""
+    if pot == "tersoff":
+        return 342.0 * in_range + 53.0 * triplets
+    return 20.0 * listed + 178.0 * in_range + 30.0 * triplets
+
+
+def step_bytes(listed, in_range, n, rebuild_every, fp32):
+    """Algorithmic HBM bytes of one md_nve_run step, from the same counts.
+    pair phase : x,y,z 24 + NN 4 + MASK 8 + own-half f 24 per atom; list entry 4 per listed pair; reverse
+                 slot 1 + record 32 (16 in FP32 mode) per in-range pair   (neighbour coordinates: L2-served)
+    gather+VV  : MASK 8 + own-half f 24 + v 24 + x 24 read, v 24 + x 24 written per atom; record per in-range pair
+    build      : x,y,z read twice 48 + cell-ordered copies written and read 96 + NN 4 per atom; list entry
+                 written and read 8 + reverse slot 1 per listed pair -- every `rebuild_every` steps"""
+    rec = 16.0 if fp32 else 32.0
+    pair = 60.0 * n + 4.0 * listed + (1.0 + rec) * in_range
+    gather = 128.0 * n + rec * in_range
+    build = (148.0 * n + 9.0 * listed) / rebuild_every
+    return pair + gather + build
 
 
 def measured_peaks():
@@ -94,14 +121,20 @@ def reference_sample_ncell(full_ncell, steps, warmup):
     return max(3, min(full_ncell, nc))
 
 
-def run_oracle(cfg_index, steps, warmup, ncell):
+def run_oracle(cfg_index, steps, warmup, ncell, threads=1):
+    """Oracle NVE on `ncell`^3 cells of config `cfg_index`: `warmup` untimed steps (they also provide the
+    forces), then `steps` timed ones.  threads > 1: the force evaluation on that many threads."""
     import oracle                                            # the one CPU leg allowed to use oracle/
     c = mi.make_config(cfg_index, ncell=ncell)
     K = c["max_neighbors"] if c["potential"] == "tersoff" else 40
     st = {k: c[k] for k in ("x", "y", "z", "vx", "vy", "vz", "box", "mass")}
     r = oracle.nve_run(c["potential"], c["params"], st, warmup, c["dt"], c["rebuild_every"], c["r_list"], K)
     t0 = time.perf_counter()
-    oracle.nve_run(c["potential"], c["params"], st, steps, c["dt"], c["rebuild_every"], c["r_list"], K, f=r["f"])
+    if threads > 1:
+        oracle.nve_run_threads(c["potential"], c["params"], st, steps, c["dt"], c["rebuild_every"], c["r_list"], K,
+                               threads, r["f"])
+    else:
+        oracle.nve_run(c["potential"], c["params"], st, steps, c["dt"], c["rebuild_every"], c["r_list"], K, f=r["f"])
     dt = time.perf_counter() - t0
     return c["n"], dt
 
@@ -151,165 +184,309 @@ def aggregate_value(n_per_rank, steps, world, ms_max):
     return world * n_per_rank * steps / (ms_max * 1e-3)
 
 
-def main_ours(args):
-    import torch
-    import torch.distributed as dist
+class Gpu:
+    """Device, rank and barrier shared by the measurements of one bench.py process."""
 
-    import paper_1610_03343_b200 as md
+    def __init__(self):
+        import torch
+        import torch.distributed as dist
+        self.torch, self.dist = torch, dist
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+        torch.cuda.set_device(self.local)
+        self.dev = f"cuda:{self.local}"
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=torch.device(self.dev))
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)   # > 126 MB L2
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = f"cuda:{local}"
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    def flush_l2(self):
+        """256 MiB written, then read back so that no dirty foreign lines are left to evict."""
+        self.flush.zero_()
+        self.flush.sum()
 
-    c = mi.make_config(args.config)
+    def close(self):
+        if self.world > 1:
+            self.dist.destroy_process_group()
+
+
+def kernel_name(md, nl, pot, n):
+    if pot == "sw":
+        return "k_screen+k_sw_sorted"
+    _, long_rows = md.md_neighbors_row_stats(nl)
+    return "k_screen+k_tersoff_sorted" if long_rows * 256 > n else "k_tersoff_atom"
+
+
+def measure_nve(gpu, md, cfg_index, steps, warmup, fp32, peaks, fp64_peak, with_e2e, sampler=None):
+    """K NVE steps of BASELINE config `cfg_index` as ceil(K/chunk) md_nve_run calls of one rebuild cycle each,
+    every call bracketed by its own CUDA-event pair, L2 flushed before every call outside the pairs; a second
+    pass with the library's per-kernel-kind events; one back-to-back call; optionally the host-buffer call."""
+    torch = gpu.torch
+    c = mi.make_config(cfg_index)
     pot, n, K = c["potential"], c["n"], c["max_neighbors"]
     box, mass, dt, rebuild, r_list = list(c["box"]), c["mass"], c["dt"], c["rebuild_every"], c["r_list"]
     host0 = {k: torch.from_numpy(c[k].copy()) for k in ("x", "y", "z", "vx", "vy", "vz")}
-    d = {k: v.to(dev) for k, v in host0.items()}
-    f = torch.zeros((3, n), dtype=torch.float64, device=dev)
-    pe = torch.zeros(n, dtype=torch.float64, device=dev)
+    d = {k: v.to(gpu.dev) for k, v in host0.items()}
+    f = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    pe = torch.zeros(n, dtype=torch.float64, device=gpu.dev)
     nl = md.md_neighbors_create(n, K)
-    prec = md.MD_FP32 if args.fp32 else md.MD_FP64
+    prec = md.MD_FP32 if fp32 else md.MD_FP64
 
     def run(first, nsteps, f_valid=True):
         md.md_nve_run(nl, pot, c["params"], n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], f, f_valid, pe,
                       box, mass, dt, nsteps, rebuild, r_list, precision=prec, first_step=first)
 
     run(0, 0, f_valid=False)                       # forces of the initial state
-    run(0, args.warmup)
-    step0 = args.warmup
+    run(0, warmup)
+    step0 = warmup
     max_row = md.md_neighbors_status(nl)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-
     chunk = rebuild                                # one timed call = one rebuild cycle of md_nve_run
 
     def timed_pass(profile):
-        """K steps as ceil(K/chunk) md_nve_run calls of `chunk` steps (the last one shorter), each bracketed
-        by its own CUDA-event pair; L2 flushed (256 MiB written, then read back so that no dirty foreign
-        lines are left to evict) before every call, outside the event pairs."""
         nonlocal step0
         md.md_profile_enable(nl, profile)
         md.md_profile_read(nl)
-        sizes = [min(chunk, args.steps - k) for k in range(0, args.steps, chunk)]
+        sizes = [min(chunk, steps - k) for k in range(0, steps, chunk)]
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in sizes]
-        barrier()
+        gpu.barrier()
         t0 = time.perf_counter()
         done = 0
         for k, sz in enumerate(sizes):
-            flush.zero_()                          # L2 flush between timed iterations (not timed)
-            flush.sum()
+            gpu.flush_l2()                         # L2 flush between timed iterations (not timed)
             ev[k][0].record()
             run(step0 + done, sz)
             ev[k][1].record()
             done += sz
         torch.cuda.synchronize()
         t1 = time.perf_counter()
-        barrier()
-        step0 += args.steps
+        gpu.barrier()
+        step0 += steps
         ms = sum(a.elapsed_time(b) for a, b in ev)
         kinds_ms, launches = md.md_profile_read(nl)
         md.md_profile_enable(nl, False)
         return ms, kinds_ms, launches, t0, t1
 
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.1)
+    if sampler is not None:
+        sampler.start()
+        time.sleep(0.1)
     ms_total, _, launches, t0, t1 = timed_pass(False)
-    clocks = sampler.stop(t0, t1)
-    # same loop with per-kernel-kind events (roofline of the dominant kernel)
-    ms_prof, kinds_ms, launches_prof, _, _ = timed_pass(True)
-    # back-to-back steps, one C call, no flush (what a production MD loop does)
-    barrier()
+    clocks = sampler.stop(t0, t1) if sampler is not None else None
+    ms_prof, kinds_ms, _, _, _ = timed_pass(True)  # same loop with per-kernel-kind events
+    gpu.barrier()                                  # back-to-back steps, one C call, no flush
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(); run(step0, args.steps); e1.record()
+    e0.record(); run(step0, steps); e1.record()
     torch.cuda.synchronize()
     ms_b2b = e0.elapsed_time(e1)
-    step0 += args.steps
+    step0 += steps
     md.md_neighbors_status(nl)
+    listed, in_range, triplets = md.md_pair_counts(nl)
+    kern = kernel_name(md, nl, pot, n)
     e_final = float(pe.sum())
 
-    # end to end through the C ABI with HOST (pinned) buffers: H2D + K steps + D2H inside the timed region
-    hp = {k: v.clone().pin_memory() for k, v in host0.items()}
-    hf = torch.zeros((3, n), dtype=torch.float64).pin_memory()
-    hpe = torch.zeros(n, dtype=torch.float64).pin_memory()
-    nl2 = md.md_neighbors_create(n, K)
+    e2e_ms = None
+    if with_e2e:                                   # C ABI with HOST (pinned) buffers: H2D + K steps + D2H timed
+        hp = {k: v.clone().pin_memory() for k, v in host0.items()}
+        hf = torch.zeros((3, n), dtype=torch.float64).pin_memory()
+        hpe = torch.zeros(n, dtype=torch.float64).pin_memory()
+        nl2 = md.md_neighbors_create(n, K)
 
-    def e2e_call(nsteps):
-        for k, v in host0.items():
-            hp[k].copy_(v)
-        barrier()
-        t = time.perf_counter()
-        md.md_nve_run_host(nl2, pot, c["params"], n, hp["x"], hp["y"], hp["z"], hp["vx"], hp["vy"], hp["vz"],
-                           hf, hpe, box, mass, dt, nsteps, rebuild, r_list, precision=prec)
-        return time.perf_counter() - t
-    e2e_call(max(3, args.warmup))
-    e2e_s = e2e_call(args.steps)
-    md.md_neighbors_status(nl2)
+        def e2e_call(nsteps):
+            for k, v in host0.items():
+                hp[k].copy_(v)
+            gpu.barrier()
+            t = time.perf_counter()
+            md.md_nve_run_host(nl2, pot, c["params"], n, hp["x"], hp["y"], hp["z"], hp["vx"], hp["vy"], hp["vz"],
+                               hf, hpe, box, mass, dt, nsteps, rebuild, r_list, precision=prec)
+            return time.perf_counter() - t
+        e2e_call(max(3, warmup))
+        e2e_ms = e2e_call(steps) * 1e3
+        md.md_neighbors_destroy(nl2)
+    md.md_neighbors_destroy(nl)
 
-    ms_total, ms_prof, ms_b2b, e2e_ms = max_over_ranks([ms_total, ms_prof, ms_b2b, e2e_s * 1e3], dev, world)
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return 0
+    vals = gpu_max([ms_total, ms_prof, ms_b2b, e2e_ms if e2e_ms is not None else 0.0], gpu)
+    ms_total, ms_prof, ms_b2b = vals[:3]
+    e2e_ms = vals[3] if e2e_ms is not None else None
+    world = gpu.world
+    pair_ms = kinds_ms["pair"] / steps             # one pair phase per step
+    flops = pair_flop_equiv(pot, listed, in_range, triplets)
+    achieved = flops / (pair_ms * 1e-3) / 1e12
+    nbytes = step_bytes(listed, in_range, n, rebuild, fp32)
+    hbm_peak = peaks.get("hbm_gbs")
+    hbm_gbs = nbytes / (ms_total / steps * 1e-3) / 1e9
+    return {
+        "c": c, "value": aggregate_value(n, steps, world, ms_total), "ms_per_step": ms_total / steps,
+        "ms_per_step_profiled": ms_prof / steps, "ms_b2b": ms_b2b, "e2e_ms": e2e_ms, "clocks": clocks,
+        "launches": launches, "kinds_ms": kinds_ms, "max_row": max_row, "kernel": kern, "pair_ms": pair_ms,
+        "counts": {"listed_pairs": listed, "in_range_pairs": in_range, "ordered_triplets": triplets,
+                   "listed_per_atom": listed / n, "in_range_per_atom": in_range / n,
+                   "ordered_triplets_per_atom": triplets / n},
+        "alu": {"achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s", "frac": achieved / fp64_peak,
+                "flop_equiv_per_atom": flops / n, "kernel": kern, "kernel_ms": pair_ms},
+        "hbm": {"achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s",
+                "frac": hbm_gbs / hbm_peak if hbm_peak else None, "bytes_per_atom_step": nbytes / n,
+                "what": "algorithmic bytes of a whole md_nve_run step / ms_per_step",
+                "peak_source": "MEASURED_PEAKS.json" if hbm_peak else "absent"},
+        "final_pe_per_atom": e_final / n,
+    }
 
+
+def gpu_max(values, gpu):
+    return max_over_ranks(values, gpu.dev, gpu.world)
+
+
+def measure_eval(gpu, md, cfg_index, calls, warmup, fp64_peak, peaks):
+    """Config 1's mode: ONE evaluation of energy, forces, virial and heat current per "step" (atom-evals/s).
+    Each call is bracketed by its own event pair; L2 is flushed before every call."""
+    torch = gpu.torch
+    c = mi.make_config(cfg_index)
+    pot, n, K = c["potential"], c["n"], c["max_neighbors"]
+    box = list(c["box"])
+    d = {k: torch.from_numpy(c[k]).to(gpu.dev) for k in ("x", "y", "z", "vx", "vy", "vz")}
+    pe = torch.zeros(n, dtype=torch.float64, device=gpu.dev)
+    f = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    W = torch.zeros((9, n), dtype=torch.float64, device=gpu.dev)
+    J = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    nl = md.md_neighbors_create(n, K)
+    md.md_build_neighbors(nl, n, d["x"], d["y"], d["z"], box, c["r_list"])
+    fn = md.md_tersoff_force if pot == "tersoff" else md.md_sw_force
+
+    def call():
+        fn(nl, n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], box, c["params"], md.MD_FP64,
+           pe=pe, f=f, virial=W, heat=J)
+    for _ in range(max(3, warmup)):
+        call()
+    md.md_neighbors_status(nl)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+    gpu.barrier()
+    for a, b in ev:
+        gpu.flush_l2()
+        a.record(); call(); b.record()
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    ms, = gpu_max([ms], gpu)
+    listed, in_range, triplets = md.md_pair_counts(nl)
+    md.md_neighbors_destroy(nl)
+    rec = 32.0
+    # pair kernel + k_gather with all outputs: adds list entry 4 + neighbour coordinates (L2) per in-range pair,
+    # W 72 read + 72 written, J 24, v 24, x 24, U 8 per atom (DESIGN.md section 3)
+    nbytes = (60.0 + 8.0) * n + 4.0 * listed + (1.0 + rec) * in_range + (8 + 24 + 24 + 24 + 144 + 24 + 24) * n \
+        + (rec + 4.0) * in_range
+    hbm_peak = peaks.get("hbm_gbs")
+    return {"workload": c["name"], "atoms": n, "outputs": "pe, f, virial(9), heat", "calls": calls,
+            "value": gpu.world * n * calls / (ms * 1e-3), "unit": "atom-evals/s", "us_per_eval": 1e3 * ms / calls,
+            "hbm_frac": (nbytes / (ms / calls * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None,
+            "bytes_per_atom_eval": nbytes / n, "in_range_per_atom": in_range / n}
+
+
+def summary(r):
+    """The per-config entry of the line's `configs` object."""
+    c = r["c"]
+    return {"workload": c["name"], "potential": c["potential"], "atoms": c["n"], "dt_fs": c["dt"],
+            "value": r["value"], "unit": UNIT, "ms_per_step": r["ms_per_step"],
+            "kernels_ms_per_step": {k: v / max(1, r["steps"]) for k, v in r["kinds_ms"].items()},
+            "pair_kernel": r["kernel"], "pair_ms": r["pair_ms"], "alu_frac": r["alu"]["frac"],
+            "alu_tflops": r["alu"]["achieved"], "flop_equiv_per_atom": r["alu"]["flop_equiv_per_atom"],
+            "hbm_frac": r["hbm"]["frac"], "hbm_gbs": r["hbm"]["achieved"],
+            "bytes_per_atom_step": r["hbm"]["bytes_per_atom_step"], "counts_per_atom": {
+                k: r["counts"][k] for k in ("listed_per_atom", "in_range_per_atom", "ordered_triplets_per_atom")},
+            "steps": r["steps"], "max_row_seen": r["max_row"]}
+
+
+def main_ours(args):
+    import paper_1610_03343_b200 as md
+
+    gpu = Gpu()
     peaks = measured_peaks()
     fp64_peak = md.md_probe_fp64_peak(20000)
-    n_pair = max(1, launches_prof["pair"])
-    pair_ms = kinds_ms["pair"] / n_pair
-    achieved = PAIR_FLOP_PER_ATOM[pot] * n / (pair_ms * 1e-3) / 1e12
-    _, long_rows = md.md_neighbors_row_stats(nl)
-    kern = "k_sw_pairs_cta" if pot == "sw" else ("k_tersoff_pairs_cta" if long_rows * 256 > n else "k_tersoff_atom")
-    value = aggregate_value(n, args.steps, world, ms_total)
+    if mi.CONFIGS[args.config]["steps"] == 0:                # config 1: evaluation mode
+        r = measure_eval(gpu, md, args.config, args.steps, args.warmup, fp64_peak, peaks)
+        if gpu.rank == 0:
+            print(json.dumps({"metric": "atom-evals/s (FP64 Tersoff: energy, forces, virial, heat current)",
+                              "n_gpus": gpu.world, "steps": args.steps, "warmup": args.warmup,
+                              "higher_is_better": True, "dtype": "f64", "data": "synthetic", **r}))
+        gpu.close()
+        return 0
+
+    sampler = ClockSampler(gpu.local)
+    r = measure_nve(gpu, md, args.config, args.steps, args.warmup, args.fp32, peaks, fp64_peak, True, sampler)
+    r["steps"] = args.steps
+    c, n, world = r["c"], r["c"]["n"], gpu.world
+    extra = {}
+    if not args.only_headline:
+        # the other BASELINE configs, bounded (their own length or --steps, whichever is shorter)
+        for idx, fp32 in ((2, False), (4, False), (4, True), (3, False)):
+            if idx == args.config and fp32 == args.fp32:
+                continue
+            k = min(args.steps, mi.CONFIGS[idx]["steps"])
+            q = measure_nve(gpu, md, idx, k, args.warmup, fp32, peaks, fp64_peak, False)
+            q["steps"] = k
+            extra[mi.CONFIGS[idx]["name"] + ("_fp32" if fp32 else "")] = summary(q)
+        extra["cfg1_tersoff_512_eval"] = measure_eval(gpu, md, 0, 200, args.warmup, fp64_peak, peaks)
+        extra["cfg2_size_full_output_eval"] = measure_eval(gpu, md, 1, 20, args.warmup, fp64_peak, peaks)
+    if gpu.rank != 0:
+        gpu.close()
+        return 0
+
+    kinds_ms, steps = r["kinds_ms"], args.steps
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.fp32 else "f64", "data": "synthetic",
-        "config": {"workload": c["name"], "potential": pot, "atoms_per_gpu": n, "dt_fs": dt,
-                   "rebuild_every": rebuild, "r_list": r_list, "max_neighbors": K, "max_row_seen": max_row,
+        "config": {"workload": c["name"], "potential": c["potential"], "atoms_per_gpu": n, "dt_fs": c["dt"],
+                   "rebuild_every": c["rebuild_every"], "r_list": c["r_list"], "max_neighbors": c["max_neighbors"],
+                   "max_row_seen": r["max_row"],
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "steps_per_timed_call": chunk,
-                   "l2": f"flushed (256 MiB written then read) before every timed md_nve_run call of {chunk} steps, "
-                         "outside the CUDA-event pairs"},
-        "clocks": clocks,
-        "e2e": {"value": world * n * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
-                "h2d_bytes_per_step": 6 * 8 * n / args.steps, "d2h_bytes_per_step": 10 * 8 * n / args.steps,
-                "what": f"md_nve_run_host: pinned host x,v -> device, {args.steps} steps, x,v,f,pe -> host"},
-        "gpu_launches": int(sum(launches.values())),
-        "roofline": {"bound": "alu", "kernel": kern, "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                     "frac": achieved / fp64_peak, "traffic": traffic_from_profiles(kern),
+                   "steps_per_timed_call": c["rebuild_every"],
+                   "l2": f"flushed (256 MiB written then read) before every timed md_nve_run call of "
+                         f"{c['rebuild_every']} steps, outside the CUDA-event pairs"},
+        "clocks": r["clocks"],
+        "e2e": {"value": world * n * steps / (r["e2e_ms"] * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": 6 * 8 * n / steps, "d2h_bytes_per_step": 10 * 8 * n / steps,
+                "what": f"md_nve_run_host: pinned host x,v -> device, {steps} steps, x,v,f,pe -> host"},
+        "gpu_launches": int(sum(r["launches"].values())),
+        "roofline": {"bound": "alu", "kernel": r["kernel"], "achieved": r["alu"]["achieved"], "peak": fp64_peak,
+                     "unit": "TFLOP/s", "frac": r["alu"]["frac"], "traffic": traffic_from_profiles(r["kernel"]),
                      "peak_source": "md_probe_fp64_peak (measured DFMA rate, this run); nominal "
                                     f"{FP64_NOMINAL_TFLOPS:.1f}",
-                     "flop_equiv_per_atom": PAIR_FLOP_PER_ATOM[pot], "kernel_ms": pair_ms,
+                     "flop_equiv_per_atom": r["alu"]["flop_equiv_per_atom"], "kernel_ms": r["pair_ms"],
+                     "counts_per_atom": {k: r["counts"][k] for k in ("listed_per_atom", "in_range_per_atom",
+                                                                     "ordered_triplets_per_atom")},
                      "kernel_share_of_step": kinds_ms["pair"] / max(1e-9, sum(kinds_ms.values()))},
-        "kernels_ms_per_step": {k: v / args.steps for k, v in kinds_ms.items()},
-        "ms_per_step_profiled": ms_prof / args.steps,
-        "back_to_back": {"value": world * n * args.steps / (ms_b2b * 1e-3), "unit": UNIT,
-                         "ms_per_step": ms_b2b / args.steps, "l2": "not flushed; one md_nve_run call"},
-        "hbm": {"hbm_gbs_peak": peaks.get("hbm_gbs"), "peak_source": "MEASURED_PEAKS.json" if peaks else "absent"},
-        "final_pe_per_atom": e_final / n,
+        "hbm": r["hbm"],
+        "kernels_ms_per_step": {k: v / steps for k, v in kinds_ms.items()},
+        "ms_per_step_profiled": r["ms_per_step_profiled"],
+        "back_to_back": {"value": world * n * steps / (r["ms_b2b"] * 1e-3), "unit": UNIT,
+                         "ms_per_step": r["ms_b2b"] / steps, "l2": "not flushed; one md_nve_run call"},
+        "final_pe_per_atom": r["final_pe_per_atom"],
         "paper_context": "K40 FP64 Tersoff, 512000 atoms ~ 100 X5670 cores ~ 2.7e7 atom-steps/s (PAPER.md:365-373)",
     }
+    if extra:
+        line["configs"] = extra
     if world == 1 and not args.no_cpu_baseline:
-        ncell = 40 if c["ncell"] >= 40 else c["ncell"]
-        cb_steps = 3
-        n_cb, dt_cb = run_oracle(args.config if c["ncell"] <= 40 else 1, cb_steps, 0, ncell)
+        # the oracle as it stands on this box's host cores: one full rebuild cycle (the GPU's cadence)
+        src = args.config if c["ncell"] <= 40 else 1
+        ncell = min(40, c["ncell"])
+        cb_steps = c["rebuild_every"]
+        n_cb, dt_cb = run_oracle(src, cb_steps, 0, ncell)
         line["cpu_baseline"] = {"value": n_cb * cb_steps / dt_cb, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"{n_cb} atoms of the same recipe, {cb_steps} NVE steps incl. one "
-                                          f"list build, given initial forces, 1 thread, {dt_cb:.1f} s"}
+                                "sample": f"{n_cb} atoms of the same recipe, {cb_steps} NVE steps = one rebuild "
+                                          f"cycle incl. its list build, given initial forces, 1 thread, {dt_cb:.1f} s"}
+        cores = len(os.sched_getaffinity(0))
+        if cores > 1:
+            n_ca, dt_ca = run_oracle(src, cb_steps, 0, ncell, threads=cores)
+            line["cpu_baseline_all_cores"] = {
+                "value": n_ca * cb_steps / dt_ca, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": f"same sample; force evaluation on {cores} threads over atom ranges with per-thread "
+                          f"force buffers, list build and integrator on one; {dt_ca:.1f} s"}
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    gpu.close()
     return 0
 
 
@@ -322,6 +499,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--fp32", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--only-headline", action="store_true", help="skip the `configs` summary of the other configs")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

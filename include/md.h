@@ -18,11 +18,19 @@
  *     structure-of-arrays: f[3][n], virial[9][n] (row-major ab, a from r, b from F: W_ab = -1/2 sum r^a F^b),
  *     heat[3][n].  Nothing in caller arrays is permuted.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and
- *     return without synchronising unless stated.
+ *     return without synchronising unless stated.  The force calls never wait for the device: the choice
+ *     between the Tersoff kernels uses the row statistics of the last list build whose (asynchronous)
+ *     copy to the host has arrived; only the very first force call on a handle waits for its build.
  *   - Return value: MD_OK or a negative md_status.  Argument errors are detected synchronously and
  *     have no side effects.  Conditions found on the device (a neighbour row longer than
  *     max_neighbors, a missing reverse entry, too many in-range neighbours) latch a status word in
  *     the handle; md_neighbors_status() synchronises the stream and returns it.
+ *   - Capacity limits beyond max_neighbors (all latch MD_ERR_NEIGHBOR_OVERFLOW, results are then invalid):
+ *     at most 32 neighbours of one atom inside the force range; the register Tersoff kernel's per-thread
+ *     fallback for rows longer than 4 holds 16 in-range neighbours; the sorted kernels keep the in-range
+ *     neighbours of a 128-atom tile in a shared-memory pool of 128 x 8 (Tersoff) or 128 x 12
+ *     (Stillinger-Weber) slots, of which each of the tile's four warps (atoms sorted by in-range count) takes
+ *     32 x its largest count: the four largest-per-warp counts must sum to <= 32 (Tersoff) / 48 (SW).
  *   - There is no CPU fallback: every entry point needs a CUDA device.
  */
 #ifndef MD_H_
@@ -77,7 +85,8 @@ int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than
 /* Copy the current list out / in (DEVICE int32 buffers): NN[n]; NL[max_neighbors][n] neighbour-major,
  * NL[m*n + i] = index of the m-th neighbour of atom i, rows sorted by index.
  * Import also rebuilds the reverse index; it lets a test drive the force kernels with an
- * externally built list. */
+ * externally built list.  Imported rows must be sorted by index and the list symmetric (j in row i <=> i in
+ * row j); otherwise MD_ERR_LIST_ASYMMETRIC is latched. */
 int md_neighbors_export(md_neighbors* nl, int32_t* NN, int32_t* NL, void* stream);
 int md_neighbors_import(md_neighbors* nl, int64_t n, const int32_t* NN, const int32_t* NL, void* stream);
 
@@ -121,7 +130,8 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
 
 /* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
  * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
- * synchronises.  Device buffers are owned by the handle. */
+ * synchronises.  Device buffers are owned by the handle.  Returns the latched device status (as
+ * md_neighbors_status would) since it has synchronised anyway. */
 int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                     double* x, double* y, double* z, double* vx, double* vy, double* vz,
                     double* f, double* pe, const double box[3], double mass_amu, double dt_fs,
@@ -145,6 +155,12 @@ int md_math_probe(int fn, int64_t n, const double* in, double* out, void* stream
 enum { MD_KIND_BUILD = 0, MD_KIND_PAIR = 1, MD_KIND_GATHER = 2, MD_KIND_INTEGRATE = 3, MD_N_KINDS = 4 };
 int md_profile_enable(md_neighbors* nl, int enable);
 int md_profile_read(md_neighbors* nl, double* ms, int64_t* launches);
+
+/* Diagnostic: exact integer counts over the current list and the in-range masks the LAST force call left
+ * (HOST int64 out[3]): out[0] = listed directed pairs (sum of row lengths), out[1] = directed pairs inside the
+ * force range, out[2] = ordered in-range triplets sum_i M_i (M_i - 1).  bench.py multiplies them by the
+ * per-unit operation counts of DESIGN.md section 3 to get the algorithmic work of a launch.  Synchronous. */
+int md_pair_counts(md_neighbors* nl, int64_t out[3], void* stream);
 
 /* Library version string (HOST, static storage). */
 const char* md_version(void);

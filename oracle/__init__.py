@@ -101,6 +101,50 @@ def evaluate(potential, params, x, y, z, box, NN, NL, v=None, precision="f64",
     return out
 
 
+def evaluate_threads(potential, params, x, y, z, box, NN, NL, nthreads):
+    """pe[n] and the conventional forces f[3][n] with the atoms split into `nthreads` contiguous ranges, one
+    thread each (ctypes releases the GIL), each scattering into its own force buffer (Algorithm 1 writes to j
+    and k: PAPER.md:157-161); the buffers are added afterwards.  Timing entry for bench.py's all-core
+    cpu_baseline: the per-atom functions are the single-thread oracle's, unchanged."""
+    from concurrent.futures import ThreadPoolExecutor
+    x, y, z, box = _f64(x), _f64(y), _f64(z), _f64(box)
+    n, K = x.size, NL.shape[1]
+    par = pack_params(potential, params)
+    NN = np.ascontiguousarray(NN, dtype=np.int32)
+    NL = np.ascontiguousarray(NL, dtype=np.int32)
+    pe = np.zeros(n)
+    bounds = np.linspace(0, n, nthreads + 1).astype(np.int64)
+    bufs = [np.zeros((3, n)) for _ in range(nthreads)]
+    fn = lib().oracle_evaluate_range
+
+    def work(t):
+        rc = fn(C.c_int(pot_id(potential)), _p(par), C.c_int64(n), _p(x), _p(y), _p(z), _p(box),
+                _p(NN, C.c_int32), _p(NL, C.c_int32), C.c_int(K), C.c_int64(int(bounds[t])),
+                C.c_int64(int(bounds[t + 1])), _p(pe), _p(bufs[t]))
+        if rc != 0:
+            raise RuntimeError(f"oracle_evaluate_range failed rc={rc}")
+    with ThreadPoolExecutor(nthreads) as ex:
+        list(ex.map(work, range(nthreads)))
+    f = bufs[0]
+    for b in bufs[1:]:
+        f += b
+    return pe, f
+
+
+def nve_run_threads(potential, params, state, nsteps, dt, rebuild_every, r_list, K, nthreads, f):
+    """The NVE loop of nve_run with the force evaluation on `nthreads` threads (list build and integrator stay
+    single-threaded).  `f` must hold the forces of the incoming state.  Returns the final forces."""
+    NN = NL = None
+    for s in range(nsteps):
+        vv_kick_drift(state["x"], state["y"], state["z"], state["vx"], state["vy"], state["vz"], f,
+                      state["mass"], dt, state["box"])
+        if s % rebuild_every == 0 or NN is None:
+            NN, NL = neighbors(state["x"], state["y"], state["z"], state["box"], r_list, K, method="cell")
+        _, f = evaluate_threads(potential, params, state["x"], state["y"], state["z"], state["box"], NN, NL, nthreads)
+        vv_kick(state["vx"], state["vy"], state["vz"], f, state["mass"], dt)
+    return f
+
+
 def atom_energy(potential, params, rvecs) -> float:
     """U_i from explicit relative vectors r_ij (shape [M][3]), long double inside."""
     r = np.ascontiguousarray(rvecs, dtype=np.float64)

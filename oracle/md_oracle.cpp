@@ -417,19 +417,27 @@ void sw_conventional_atom(const SWPar& pp, const Local<R>& L, int64_t i, R* F, i
 // ======================================================================
 enum { POT_TERSOFF = 0, POT_SW = 1 };
 
+// Atoms i0 <= i < i1 only (the whole system: 0, n).  A proper sub-range serves bench.py's all-core timing
+// entry: the same per-atom functions, called by several threads on disjoint ranges, each with its own
+// force buffer because Algorithm 1 scatters to j and k; the per-pair outputs (f_pair,
+// virial, heat, P_out), which need every atom's P, are then not available and must be NULL.
 template <class R>
 int evaluate(int pot, const void* par, int64_t n, const double* x, const double* y, const double* z,
              const double* vx, const double* vy, const double* vz, const double* box,
              const int32_t* NN, const int32_t* NL, int K,
-             double* pe, double* f_conv, double* f_pair, double* virial, double* heat, double* P_out) {
+             double* pe, double* f_conv, double* f_pair, double* virial, double* heat, double* P_out,
+             int64_t i0, int64_t i1) {
     const TersoffPar* tp = (const TersoffPar*)par;
     const SWPar* sp = (const SWPar*)par;
     const double r_force = pot == POT_TERSOFF ? tp->S : sp->a * sp->sigma;
+    const bool whole = i0 == 0 && i1 == n;
+    const bool need_P = P_out || f_pair || virial || heat;
+    if (need_P && !whole) return -4;
     std::vector<R> F((size_t)3 * n, R(0));
-    std::vector<R> P((size_t)3 * n * K, R(0));     // P[(i*K+m)*3+a] = dU_i/dr_ij^a, j = NL[i*K+m]
+    std::vector<R> P(need_P ? (size_t)3 * n * K : (size_t)3 * K, R(0));   // P[(i*K+m)*3+a] = dU_i/dr_ij^a, j = NL[i*K+m]
     Local<R> L;
     std::vector<Dual<R>> vxr(MAXM), vyr(MAXM), vzr(MAXM);
-    for (int64_t i = 0; i < n; ++i) {
+    for (int64_t i = i0; i < i1; ++i) {
         if (!gather_local<R>(L, i, x, y, z, box, NN, NL, K, r_force)) return -2;
         // conventional forces (Algorithm 1)
         if (pot == POT_TERSOFF) tersoff_conventional_atom<R>(*tp, L, i, F.data(), n);
@@ -445,11 +453,13 @@ int evaluate(int pot, const void* par, int64_t n, const double* x, const double*
             ? tersoff_Ui<Dual<R>, R>(*tp, L.M, vxr.data(), vyr.data(), vzr.data())
             : sw_Ui<Dual<R>, R>(*sp, L.M, vxr.data(), vyr.data(), vzr.data());
         if (pe) pe[i] = (double)Ui.v;
+        const size_t row = need_P ? (size_t)i * K : 0;     // without per-pair outputs one row of scratch is reused
         for (int a = 0; a < L.M; ++a)
-            for (int q = 0; q < 3; ++q) P[((size_t)i * K + L.slot[a]) * 3 + q] = Ui.g[3 * a + q];
+            for (int q = 0; q < 3; ++q) P[(row + L.slot[a]) * 3 + q] = Ui.g[3 * a + q];
     }
     if (f_conv) for (size_t q = 0; q < (size_t)3 * n; ++q) f_conv[q] = (double)F[q];
     if (P_out) for (size_t q = 0; q < (size_t)3 * n * K; ++q) P_out[q] = (double)P[q];
+    if (!need_P) return 0;
     // per-atom outputs, Eqs. (28)-(30)
     for (int64_t i = 0; i < n; ++i) {
         R fp[3] = {0, 0, 0}, W[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, J[3] = {0, 0, 0};
@@ -527,9 +537,20 @@ int oracle_evaluate(int pot, const double* par, int precision, int64_t n,
                     double* pe, double* f_conv, double* f_pair, double* virial, double* heat, double* P_out) {
     if (precision == 1)
         return evaluate<long double>(pot, par, n, x, y, z, vx, vy, vz, box, NN, NL, K,
-                                     pe, f_conv, f_pair, virial, heat, P_out);
+                                     pe, f_conv, f_pair, virial, heat, P_out, 0, n);
     return evaluate<double>(pot, par, n, x, y, z, vx, vy, vz, box, NN, NL, K,
-                            pe, f_conv, f_pair, virial, heat, P_out);
+                            pe, f_conv, f_pair, virial, heat, P_out, 0, n);
+}
+
+// U_i (pe[i], i0 <= i < i1; other entries untouched) and the conventional forces these atoms' terms scatter
+// (f_conv[3][n], overwritten: zero except where atoms of the range, their neighbours and their neighbours'
+// partners receive a contribution).  For the threaded timing entry of bench.py; see evaluate().
+int oracle_evaluate_range(int pot, const double* par, int64_t n, const double* x, const double* y, const double* z,
+                          const double* box, const int32_t* NN, const int32_t* NL, int K,
+                          int64_t i0, int64_t i1, double* pe, double* f_conv) {
+    if (i0 < 0 || i1 > n || i0 > i1) return -5;
+    return evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN, NL, K,
+                            pe, f_conv, nullptr, nullptr, nullptr, nullptr, i0, i1);
 }
 
 // U_i of one atom from explicit relative vectors (for the finite-difference pin of P_ij)
@@ -561,7 +582,7 @@ int oracle_nve_run(int pot, const double* par, int64_t n, double* x, double* y, 
     if (!f_valid) {
         if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
         int rc = evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
-                                  pe_use, f, nullptr, nullptr, nullptr, nullptr);
+                                  pe_use, f, nullptr, nullptr, nullptr, nullptr, 0, n);
         if (rc) return rc;
     }
     for (int s = 0; s < nsteps; ++s) {
@@ -570,7 +591,7 @@ int oracle_nve_run(int pot, const double* par, int64_t n, double* x, double* y, 
             if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
         f_valid = 1;
         int rc = evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
-                                  pe_use, f, nullptr, nullptr, nullptr, nullptr);
+                                  pe_use, f, nullptr, nullptr, nullptr, nullptr, 0, n);
         if (rc) return rc;
         vv_kick(n, vx, vy, vz, f, mass, dt);
         if (pe_trace) { long double s2 = 0; for (int64_t i = 0; i < n; ++i) s2 += pe_use[i]; pe_trace[s] = (double)s2; }

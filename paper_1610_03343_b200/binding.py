@@ -39,7 +39,7 @@ class md_sw_params(C.Structure):
 EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neighbors_status",
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
-           "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats")
+           "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts")
 
 _lib = None
 
@@ -219,6 +219,14 @@ def md_probe_fp64_peak(iters=20000, stream=None) -> float:
     t = C.c_double(0.0)
     _check(load().md_probe_fp64_peak(C.c_int(iters), C.byref(t), _stream(stream)), "md_probe_fp64_peak")
     return t.value
+
+
+def md_pair_counts(nl, stream=None):
+    """(listed directed pairs, in-range directed pairs, ordered in-range triplets) of the current list and the
+    masks the last force call left.  Synchronises."""
+    out = (C.c_int64 * 3)()
+    _check(load().md_pair_counts(nl._h, out, _stream(stream)), "md_pair_counts")
+    return int(out[0]), int(out[1]), int(out[2])
 
 
 MATH_FN = {"exp": 0, "log": 1, "rcp": 2, "rsqrt": 3, "sin": 4, "cos": 5}

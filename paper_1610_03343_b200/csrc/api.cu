@@ -328,6 +328,12 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
     return md_neighbors_status(nl, nullptr, stream);
 }
 
+int md_pair_counts(md_neighbors* nl, int64_t out[3], void* stream) {
+    if (!nl || !out) return MD_ERR_ARG;
+    if (nl->n == 0) { out[0] = out[1] = out[2] = 0; return MD_OK; }
+    return md_launch_pair_counts(nl, out, (cudaStream_t)stream);
+}
+
 int md_probe_fp64_peak(int iters, double* tflops, void* stream) {
     if (iters < 1 || !tflops) return MD_ERR_ARG;
     return md_launch_probe_fp64(iters, tflops, (cudaStream_t)stream);

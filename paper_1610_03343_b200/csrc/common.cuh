@@ -128,3 +128,4 @@ int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, d
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s);
 const double* md_math_tables();   // device tables of fastmath.cuh for the current device (nullptr on failure)
 int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);
+int md_launch_pair_counts(md_neighbors* nl, int64_t out[3], cudaStream_t s);

@@ -46,3 +46,34 @@ int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s) {
     *tflops = flops / ((double)best * 1e-3) / 1e12;
     return MD_OK;
 }
+
+// ---- md_pair_counts: listed pairs, in-range pairs, ordered in-range triplets (exact integers) -------------
+namespace {
+__global__ void k_pair_counts(int64_t n, const int32_t* __restrict__ NN, const unsigned long long* __restrict__ MASK,
+                              unsigned long long* __restrict__ out) {
+    unsigned long long a = 0, b = 0, c = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const unsigned long long M = (unsigned long long)__popcll(MASK[i]);
+        a += (unsigned long long)NN[i]; b += M; c += M * (M - (M ? 1 : 0));
+    }
+    for (int d = 16; d > 0; d >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, d); b += __shfl_down_sync(0xffffffffu, b, d);
+        c += __shfl_down_sync(0xffffffffu, c, d);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&out[0], a); atomicAdd(&out[1], b); atomicAdd(&out[2], c); }
+}
+}  // namespace
+
+int md_launch_pair_counts(md_neighbors* nl, int64_t out[3], cudaStream_t s) {
+    unsigned long long* d = nullptr;
+    if (cudaMalloc(&d, 3 * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+    cudaMemsetAsync(d, 0, 3 * sizeof(unsigned long long), s);
+    k_pair_counts<<<592, 256, 0, s>>>(nl->n, nl->NN, nl->MASK, d);
+    unsigned long long h[3] = {0, 0, 0};
+    cudaError_t e = cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d);
+    if (e != cudaSuccess) return MD_ERR_CUDA;
+    for (int k = 0; k < 3; ++k) out[k] = (int64_t)h[k];
+    return MD_OK;
+}

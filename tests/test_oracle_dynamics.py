@@ -174,3 +174,15 @@ def test_generator_is_counter_based_and_has_the_stated_statistics():
     assert abs(sv - 2.980140e-3) < 1e-8
     v = np.concatenate([c["vx"], c["vy"], c["vz"]])
     assert abs(v.std() / sv - 1.0) < 0.06
+
+
+def test_threaded_evaluation_equals_single_thread():
+    """bench.py's all-core timing entry splits the atoms over threads; it must give what the oracle gives."""
+    s = mi.silicon_crystal(3, 0.1, 800.0, 5)
+    for pot, K in (("tersoff", 16), ("sw", 40)):
+        par = mi.TERSOFF_SI_C if pot == "tersoff" else mi.SW_SI
+        NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list(pot), K)
+        ref = oracle.evaluate(pot, par, s["x"], s["y"], s["z"], s["box"], NN, NL, want=("pe", "f"))
+        pe, f = oracle.evaluate_threads(pot, par, s["x"], s["y"], s["z"], s["box"], NN, NL, 3)
+        assert (pe == ref["pe"]).all()
+        assert np.abs(f - ref["f"]).max() <= 1e-13 * np.abs(ref["f"]).max()
