@@ -26,6 +26,7 @@ KB_EV_PER_K = 8.617333262e-5          # Boltzmann constant, eV/K (CODATA 2018)
 # KAPPA = e / (u * 1e10 * 1e... ) = 1.602176634e-19 / 1.66053906660e-27 * 1e-10 (m->A: 1e20, s->fs: 1e-30)
 KAPPA = 9.648533215665e-3
 SI_MASS_AMU = 28.0855
+C_MASS_AMU = 12.011
 SI_LATTICE_A = 5.43
 
 _BASIS = np.array(
@@ -103,11 +104,40 @@ def silicon_crystal(ncell: int, sigma_disp: float, temperature: float, seed: int
     }
 
 
+def zincblende_crystal(ncell: int, a: float, sigma_disp: float, temperature: float, seed: int,
+                       masses=(SI_MASS_AMU, C_MASS_AMU)) -> dict:
+    """Zinc-blende AB crystal (the diamond sites of `diamond_lattice`: basis 0-3 = element 0, basis 4-7 =
+    element 1), seeded displacements and per-element Maxwell-Boltzmann velocities; `types` int32 [n]."""
+    x, y, z, L = diamond_lattice(ncell, a)
+    n = x.size
+    types = ((np.arange(n) % 8) >= 4).astype(np.int32)
+    if sigma_disp > 0.0:
+        d = normal_deviates(seed, STREAM_DISP, 3 * n).reshape(n, 3)
+        x = x + sigma_disp * d[:, 0]; y = y + sigma_disp * d[:, 1]; z = z + sigma_disp * d[:, 2]
+    x = wrap(x, L); y = wrap(y, L); z = wrap(z, L)
+    m = np.asarray(masses, dtype=np.float64)[types]
+    sv = np.sqrt(KB_EV_PER_K * temperature / m * KAPPA) if temperature > 0 else np.zeros(n)
+    g = normal_deviates(seed, STREAM_VEL, 3 * n).reshape(n, 3) * sv[:, None]
+    g = g - (g * m[:, None]).sum(axis=0, keepdims=True) / m.sum()       # zero total momentum
+    return {"n": n, "box": np.array([L, L, L], dtype=np.float64), "types": types, "mass": m,
+            "x": np.ascontiguousarray(x), "y": np.ascontiguousarray(y), "z": np.ascontiguousarray(z),
+            "vx": np.ascontiguousarray(g[:, 0]), "vy": np.ascontiguousarray(g[:, 1]),
+            "vz": np.ascontiguousarray(g[:, 2])}
+
+
 # --- potential parameter sets (BASELINE.json configs) -----------------------
 TERSOFF_SI_C = dict(A=1830.8, B=471.18, lam=2.4799, mu=1.7322, beta=1.1e-6, n=0.78734,
                     c=100390.0, d=16.217, h=-0.59825, R=2.7, S=3.0)
 SW_SI = dict(epsilon=2.1683, sigma=2.0951, a=1.80, lam=21.0, gamma=1.20,
              A=7.049556277, B=0.6022245584, p=4.0, q=0.0, cos0=-1.0 / 3.0)
+
+# Tersoff's multicomponent parameter sets (J. Tersoff, Phys. Rev. B 39, 5566 (1989), Table I): carbon and
+# silicon (the silicon column is the Si(C) set above), chi_Si-C = 0.9776; element order: 0 = Si, 1 = C.
+TERSOFF_C = dict(A=1393.6, B=346.74, lam=3.4879, mu=2.2119, beta=1.5724e-7, n=0.72751,
+                 c=38049.0, d=4.3484, h=-0.57058, R=1.8, S=2.1)
+TERSOFF_SIC_ELEMENTS = [TERSOFF_SI_C, TERSOFF_C]
+TERSOFF_SIC_CHI = [[1.0, 0.9776], [0.9776, 1.0]]
+SIC_LATTICE_A = 4.32
 
 SKIN = 0.5
 # BASELINE.json configs 1..5 (index 0..4).  r_list = r_force + SKIN.

@@ -145,6 +145,56 @@ def nve_run_threads(potential, params, state, nsteps, dt, rebuild_every, r_list,
     return f
 
 
+def pack_multi(elements, chi) -> np.ndarray:
+    """Parameter blob of the multi-element Tersoff form: elements = list of per-element dicts (keys as
+    TERSOFF_SI_C), chi = nt x nt matrix (chi_ii = 1)."""
+    nt = len(elements)
+    blob = [float(nt)]
+    for e in elements:
+        blob += [float(e[k]) for k in _TERSOFF_ORDER]
+    blob += [float(v) for v in np.asarray(chi, dtype=np.float64).reshape(-1)]
+    return np.array(blob, dtype=np.float64)
+
+
+def evaluate_multi(elements, chi, types, x, y, z, box, NN, NL, v=None, precision="f64",
+                   want=("pe", "f", "f_pair", "virial", "heat")):
+    """evaluate() for the multi-element Tersoff form; types[n] int32 in 0..nt-1."""
+    x, y, z, box = _f64(x), _f64(y), _f64(z), _f64(box)
+    n, K = x.size, NL.shape[1]
+    par = pack_multi(elements, chi)
+    types = np.ascontiguousarray(types, dtype=np.int32)
+    out = {}
+
+    def alloc(name, shape):
+        if name in want:
+            out[name] = np.zeros(shape, dtype=np.float64)
+            return out[name]
+        return None
+    pe = alloc("pe", n); f = alloc("f", (3, n)); fp = alloc("f_pair", (3, n))
+    W = alloc("virial", (9, n)); J = alloc("heat", (3, n)) if v is not None else None
+    P = alloc("P", (n, K, 3))
+    vx = vy = vz = None
+    if v is not None:
+        vx, vy, vz = (_f64(c) for c in v)
+    rc = lib().oracle_evaluate_multi(_p(par), C.c_int(1 if precision == "f80" else 0), C.c_int64(n),
+                                     _p(x), _p(y), _p(z), _p(vx), _p(vy), _p(vz), _p(box), _p(types, C.c_int32),
+                                     _p(np.ascontiguousarray(NN, dtype=np.int32), C.c_int32),
+                                     _p(np.ascontiguousarray(NL, dtype=np.int32), C.c_int32), C.c_int(K),
+                                     _p(pe), _p(f), _p(fp), _p(W), _p(J), _p(P))
+    if rc != 0:
+        raise RuntimeError(f"oracle_evaluate_multi failed rc={rc}")
+    return out
+
+
+def atom_energy_multi(elements, chi, ti, tj, rvecs) -> float:
+    r = np.ascontiguousarray(rvecs, dtype=np.float64)
+    rx, ry, rz = (np.ascontiguousarray(r[:, a]) for a in range(3))
+    tj = np.ascontiguousarray(tj, dtype=np.int32)
+    lib().oracle_atom_energy_multi.restype = C.c_double
+    return lib().oracle_atom_energy_multi(_p(pack_multi(elements, chi)), C.c_int(ti), C.c_int(r.shape[0]),
+                                          _p(tj, C.c_int32), _p(rx), _p(ry), _p(rz))
+
+
 def atom_energy(potential, params, rvecs) -> float:
     """U_i from explicit relative vectors r_ij (shape [M][3]), long double inside."""
     r = np.ascontiguousarray(rvecs, dtype=np.float64)

@@ -18,6 +18,8 @@
 //             differentiation (dual numbers) of the plain function U_i({r_ij}),
 //             so no hand-derived formula is shared with the GPU kernels.
 //  * W_i, J_i : Eqs. (29), (30), from P_ij.
+//  * multi-element Tersoff ("more than one type of atom"): Tersoff's multicomponent form,
+//             DESIGN.md reading A17 (per-element parameters, mixing rules, chi_ij); functions tersoff_multi_*.
 //  * SW     : not written out in the paper (Ref. [18]); standard
 //             Stillinger-Weber form, readings A6/S1-S2.
 //  * neighbour predicate, minimum image: DESIGN.md reading A7.
@@ -216,6 +218,63 @@ T sw_Ui(const SWPar& pp, int M, const T* rx, const T* ry, const T* rz) {
 }
 
 // ======================================================================
+//  Multi-element Tersoff (reading A17 = Tersoff's multicomponent formulation):
+//    U_i   = 1/2 sum_j f_C(r_ij; R_ij, S_ij) [ A_ij exp(-lambda_ij r_ij) - b_ij B_ij exp(-mu_ij r_ij) ]
+//    b_ij  = chi_ij (1 + beta_i^n_i zeta_ij^n_i)^(-1/(2 n_i))
+//    zeta_ij = sum_{k != j} f_C(r_ik; R_ik, S_ik) g_i(theta_ijk),  g_i with c_i, d_i, h_i of the CENTRAL atom
+//    mixing: lambda_ij, mu_ij arithmetic means; A_ij, B_ij, R_ij, S_ij geometric means; chi_ii = 1.
+// ======================================================================
+constexpr int MAXT = 4;
+struct TersoffMultiPar {
+    int nt;
+    TersoffPar el[MAXT];
+    double chi[MAXT][MAXT];
+};
+// blob layout (ctypes): [nt, then nt x 11 element parameters, then nt x nt chi (row-major)]
+inline TersoffMultiPar unpack_multi(const double* blob) {
+    TersoffMultiPar p;
+    p.nt = (int)blob[0];
+    for (int t = 0; t < p.nt; ++t) std::memcpy(&p.el[t], blob + 1 + 11 * t, sizeof(TersoffPar));
+    for (int a = 0; a < p.nt; ++a)
+        for (int b = 0; b < p.nt; ++b) p.chi[a][b] = blob[1 + 11 * p.nt + a * p.nt + b];
+    return p;
+}
+struct MixedPair { double A, B, lam, mu, R, S, chi; };
+inline MixedPair mix(const TersoffMultiPar& p, int a, int b) {
+    MixedPair m;
+    m.A = std::sqrt(p.el[a].A * p.el[b].A); m.B = std::sqrt(p.el[a].B * p.el[b].B);
+    m.lam = 0.5 * (p.el[a].lambda + p.el[b].lambda); m.mu = 0.5 * (p.el[a].mu + p.el[b].mu);
+    m.R = std::sqrt(p.el[a].R * p.el[b].R); m.S = std::sqrt(p.el[a].S * p.el[b].S);
+    m.chi = p.chi[a][b];
+    return m;
+}
+
+// U_i as a plain function of the M relative vectors r_ij; ti = type of i, tj[a] = type of neighbour a.
+// Neighbours beyond their pair's S contribute nothing (f_C = 0), so the caller may pass every listed one.
+template <class T, class R>
+T tersoff_multi_Ui(const TersoffMultiPar& pp, int ti, int M, const int* tj, const T* rx, const T* ry, const T* rz) {
+    const TersoffPar& ci = pp.el[ti];
+    std::vector<T> r(M);
+    for (int j = 0; j < M; ++j) r[j] = sqrt(rx[j] * rx[j] + ry[j] * ry[j] + rz[j] * rz[j]);
+    T U = r.empty() ? T() : r[0] * R(0);
+    for (int j = 0; j < M; ++j) {
+        const MixedPair mj = mix(pp, ti, tj[j]);
+        T zeta = r[j] * R(0);
+        for (int k = 0; k < M; ++k) {
+            if (k == j) continue;
+            const MixedPair mk = mix(pp, ti, tj[k]);
+            const T cs = (rx[j] * rx[k] + ry[j] * ry[k] + rz[j] * rz[k]) / (r[j] * r[k]);
+            zeta = zeta + tersoff_fc<T, R>(r[k], R(mk.R), R(mk.S)) * tersoff_g<T, R>(cs, R(ci.c), R(ci.d), R(ci.h));
+        }
+        const T b = R(mj.chi) * tersoff_b<T, R>(zeta, R(ci.beta), R(ci.n));
+        const T fR = R(mj.A) * exp(r[j] * R(-mj.lam));
+        const T fA = R(mj.B) * exp(r[j] * R(-mj.mu));
+        U = U + R(0.5) * (tersoff_fc<T, R>(r[j], R(mj.R), R(mj.S)) * (fR - b * fA));
+    }
+    return U;
+}
+
+// ======================================================================
 //  Neighbour lists (predicate: DESIGN.md reading A7)
 // ======================================================================
 // strict d2 < r_list^2 with d2 = fma(dz,dz, fma(dy,dy, dx*dx)), dx = min_image(xj - xi)
@@ -299,12 +358,14 @@ template <class R> struct Local {
     int M = 0;
     int slot[MAXM];        // position m in row i of the list
     int32_t idx[MAXM];     // atom index j
+    int type[MAXM];        // element of j (multi-element Tersoff; 0 otherwise)
     R rx[MAXM], ry[MAXM], rz[MAXM], r[MAXM];
 };
 
 template <class R>
 bool gather_local(Local<R>& loc, int64_t i, const double* x, const double* y, const double* z,
-                  const double* box, const int32_t* NN, const int32_t* NL, int K, double r_force) {
+                  const double* box, const int32_t* NN, const int32_t* NL, int K, double r_force,
+                  const int32_t* types = nullptr) {
     loc.M = 0;
     for (int m = 0; m < NN[i]; ++m) {
         const int32_t j = NL[i * K + m];
@@ -316,6 +377,7 @@ bool gather_local(Local<R>& loc, int64_t i, const double* x, const double* y, co
         if (loc.M >= MAXM) return false;
         const int a = loc.M++;
         loc.slot[a] = m; loc.idx[a] = j; loc.rx[a] = dx; loc.ry[a] = dy; loc.rz[a] = dz; loc.r[a] = r;
+        loc.type[a] = types ? types[j] : 0;
     }
     return true;
 }
@@ -369,6 +431,53 @@ void tersoff_conventional_atom(const TersoffPar& pp, const Local<R>& L, int64_t 
     }
 }
 
+// Algorithm 1 for the multi-element form: the same scatter, with the pair's mixed parameters in f_C, f_R, f_A
+// (pair i-j for the bond, pair i-k inside zeta) and the central atom's in g and b.
+template <class R>
+void tersoff_multi_conventional_atom(const TersoffMultiPar& pp, int ti, const Local<R>& L, int64_t i, R* F, int64_t n) {
+    const TersoffPar& ci = pp.el[ti];
+    const R beta = ci.beta, nn = ci.n, c = ci.c, d = ci.d, h = ci.h;
+    for (int ja = 0; ja < L.M; ++ja) {
+        const MixedPair mj = mix(pp, ti, L.type[ja]);
+        const int64_t j = L.idx[ja];
+        const R rij = L.r[ja];
+        const R ex = L.rx[ja] / rij, ey = L.ry[ja] / rij, ez = L.rz[ja] / rij;
+        const R fc = tersoff_fc<R, R>(rij, R(mj.R), R(mj.S)), fcp = tersoff_fc_prime<R>(rij, R(mj.R), R(mj.S));
+        const R fR = R(mj.A) * std::exp(-R(mj.lam) * rij), fA = R(mj.B) * std::exp(-R(mj.mu) * rij);
+        R zeta = 0;
+        for (int ka = 0; ka < L.M; ++ka) {
+            if (ka == ja) continue;
+            const MixedPair mk = mix(pp, ti, L.type[ka]);
+            const R cs = (L.rx[ja] * L.rx[ka] + L.ry[ja] * L.ry[ka] + L.rz[ja] * L.rz[ka]) / (rij * L.r[ka]);
+            zeta += tersoff_fc<R, R>(L.r[ka], R(mk.R), R(mk.S)) * tersoff_g<R, R>(cs, c, d, h);
+        }
+        const R b = R(mj.chi) * tersoff_b<R, R>(zeta, beta, nn), bp = R(mj.chi) * tersoff_b_prime<R>(zeta, beta, nn);
+        const R D = R(0.5) * ((fcp * fR - R(mj.lam) * fc * fR) - b * (fcp * fA - R(mj.mu) * fc * fA));
+        F[0 * n + i] += D * ex; F[1 * n + i] += D * ey; F[2 * n + i] += D * ez;
+        F[0 * n + j] -= D * ex; F[1 * n + j] -= D * ey; F[2 * n + j] -= D * ez;
+        const R qp = R(0.5) * fc * fA * bp;
+        for (int ka = 0; ka < L.M; ++ka) {
+            if (ka == ja) continue;
+            const MixedPair mk = mix(pp, ti, L.type[ka]);
+            const int64_t k = L.idx[ka];
+            const R rik = L.r[ka];
+            const R kx = L.rx[ka] / rik, ky = L.ry[ka] / rik, kz = L.rz[ka] / rik;
+            const R cs = ex * kx + ey * ky + ez * kz;
+            const R fck = tersoff_fc<R, R>(rik, R(mk.R), R(mk.S)), fckp = tersoff_fc_prime<R>(rik, R(mk.R), R(mk.S));
+            const R g = tersoff_g<R, R>(cs, c, d, h), gp = tersoff_g_prime<R>(cs, c, d, h);
+            const R ajx = fck * gp * (kx - cs * ex) / rij, ajy = fck * gp * (ky - cs * ey) / rij,
+                    ajz = fck * gp * (kz - cs * ez) / rij;
+            const R ckx = fckp * g * kx + fck * gp * (ex - cs * kx) / rik,
+                    cky = fckp * g * ky + fck * gp * (ey - cs * ky) / rik,
+                    ckz = fckp * g * kz + fck * gp * (ez - cs * kz) / rik;
+            F[0 * n + j] += qp * ajx; F[1 * n + j] += qp * ajy; F[2 * n + j] += qp * ajz;
+            F[0 * n + k] += qp * ckx; F[1 * n + k] += qp * cky; F[2 * n + k] += qp * ckz;
+            F[0 * n + i] -= qp * (ajx + ckx); F[1 * n + i] -= qp * (ajy + cky);
+            F[2 * n + i] -= qp * (ajz + ckz);
+        }
+    }
+}
+
 template <class R> R sw_V2_prime(const SWPar& pp, R r) {
     const R eps = pp.epsilon, sg = pp.sigma, rc = pp.a * pp.sigma, p = pp.p, q = pp.q;
     const R sp = std::pow(sg / r, p), sq = std::pow(sg / r, q);
@@ -415,7 +524,7 @@ void sw_conventional_atom(const SWPar& pp, const Local<R>& L, int64_t i, R* F, i
 // ======================================================================
 //  One evaluation: U_i, conventional F_i, P_ij (AD), pairwise F_i, W_i, J_i
 // ======================================================================
-enum { POT_TERSOFF = 0, POT_SW = 1 };
+enum { POT_TERSOFF = 0, POT_SW = 1, POT_TERSOFF_MULTI = 2 };
 
 // Atoms i0 <= i < i1 only (the whole system: 0, n).  A proper sub-range serves bench.py's all-core timing
 // entry: the same per-atom functions, called by several threads on disjoint ranges, each with its own
@@ -426,10 +535,18 @@ int evaluate(int pot, const void* par, int64_t n, const double* x, const double*
              const double* vx, const double* vy, const double* vz, const double* box,
              const int32_t* NN, const int32_t* NL, int K,
              double* pe, double* f_conv, double* f_pair, double* virial, double* heat, double* P_out,
-             int64_t i0, int64_t i1) {
+             int64_t i0, int64_t i1, const int32_t* types = nullptr) {
     const TersoffPar* tp = (const TersoffPar*)par;
     const SWPar* sp = (const SWPar*)par;
-    const double r_force = pot == POT_TERSOFF ? tp->S : sp->a * sp->sigma;
+    TersoffMultiPar mp;
+    double r_force = 0;
+    if (pot == POT_TERSOFF) r_force = tp->S;
+    else if (pot == POT_SW) r_force = sp->a * sp->sigma;
+    else {                                                   // every pair inside the largest S; f_C sorts out the rest
+        if (!types) return -6;
+        mp = unpack_multi((const double*)par);
+        for (int t = 0; t < mp.nt; ++t) r_force = std::max(r_force, mp.el[t].S);
+    }
     const bool whole = i0 == 0 && i1 == n;
     const bool need_P = P_out || f_pair || virial || heat;
     if (need_P && !whole) return -4;
@@ -438,10 +555,11 @@ int evaluate(int pot, const void* par, int64_t n, const double* x, const double*
     Local<R> L;
     std::vector<Dual<R>> vxr(MAXM), vyr(MAXM), vzr(MAXM);
     for (int64_t i = i0; i < i1; ++i) {
-        if (!gather_local<R>(L, i, x, y, z, box, NN, NL, K, r_force)) return -2;
+        if (!gather_local<R>(L, i, x, y, z, box, NN, NL, K, r_force, types)) return -2;
         // conventional forces (Algorithm 1)
         if (pot == POT_TERSOFF) tersoff_conventional_atom<R>(*tp, L, i, F.data(), n);
-        else sw_conventional_atom<R>(*sp, L, i, F.data(), n);
+        else if (pot == POT_SW) sw_conventional_atom<R>(*sp, L, i, F.data(), n);
+        else tersoff_multi_conventional_atom<R>(mp, types[i], L, i, F.data(), n);
         // U_i and P_ij = dU_i/dr_ij by forward-mode AD of the plain U_i({r_ij})
         const int nv = 3 * L.M;
         for (int a = 0; a < L.M; ++a) {
@@ -451,7 +569,8 @@ int evaluate(int pot, const void* par, int64_t n, const double* x, const double*
         }
         Dual<R> Ui = pot == POT_TERSOFF
             ? tersoff_Ui<Dual<R>, R>(*tp, L.M, vxr.data(), vyr.data(), vzr.data())
-            : sw_Ui<Dual<R>, R>(*sp, L.M, vxr.data(), vyr.data(), vzr.data());
+            : pot == POT_SW ? sw_Ui<Dual<R>, R>(*sp, L.M, vxr.data(), vyr.data(), vzr.data())
+            : tersoff_multi_Ui<Dual<R>, R>(mp, types[i], L.M, L.type, vxr.data(), vyr.data(), vzr.data());
         if (pe) pe[i] = (double)Ui.v;
         const size_t row = need_P ? (size_t)i * K : 0;     // without per-pair outputs one row of scratch is reused
         for (int a = 0; a < L.M; ++a)
@@ -540,6 +659,26 @@ int oracle_evaluate(int pot, const double* par, int precision, int64_t n,
                                      pe, f_conv, f_pair, virial, heat, P_out, 0, n);
     return evaluate<double>(pot, par, n, x, y, z, vx, vy, vz, box, NN, NL, K,
                             pe, f_conv, f_pair, virial, heat, P_out, 0, n);
+}
+
+// Multi-element Tersoff (pot = 2): par = [nt, nt x 11 element parameters, nt x nt chi], types[n] in 0..nt-1.
+int oracle_evaluate_multi(const double* par, int precision, int64_t n,
+                          const double* x, const double* y, const double* z,
+                          const double* vx, const double* vy, const double* vz, const double* box,
+                          const int32_t* types, const int32_t* NN, const int32_t* NL, int K,
+                          double* pe, double* f_conv, double* f_pair, double* virial, double* heat, double* P_out) {
+    if (precision == 1)
+        return evaluate<long double>(POT_TERSOFF_MULTI, par, n, x, y, z, vx, vy, vz, box, NN, NL, K,
+                                     pe, f_conv, f_pair, virial, heat, P_out, 0, n, types);
+    return evaluate<double>(POT_TERSOFF_MULTI, par, n, x, y, z, vx, vy, vz, box, NN, NL, K,
+                            pe, f_conv, f_pair, virial, heat, P_out, 0, n, types);
+}
+// U_i of one atom of element ti from explicit relative vectors and neighbour elements (finite-difference pin)
+double oracle_atom_energy_multi(const double* par, int ti, int M, const int32_t* tj, const double* rx,
+                                const double* ry, const double* rz) {
+    std::vector<long double> a(rx, rx + M), b(ry, ry + M), c(rz, rz + M);
+    std::vector<int> t(tj, tj + M);
+    return (double)tersoff_multi_Ui<long double, long double>(unpack_multi(par), ti, M, t.data(), a.data(), b.data(), c.data());
 }
 
 // U_i (pe[i], i0 <= i < i1; other entries untouched) and the conventional forces these atoms' terms scatter
