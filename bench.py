@@ -385,6 +385,42 @@ def measure_eval(gpu, md, cfg_index, calls, warmup, fp64_peak, peaks):
             "bytes_per_atom_eval": nbytes / n, "in_range_per_atom": in_range / n}
 
 
+def measure_multi_eval(gpu, md, calls, warmup, peaks):
+    """Multi-element Tersoff: full-output evaluations of a 512 000-atom 3C-SiC crystal
+    (zinc-blende, a = 4.32 A, sigma 0.05 A, 300 K), list cut-off 3.0 + 0.5 A, in atom-evals/s."""
+    torch = gpu.torch
+    s = mi.zincblende_crystal(40, mi.SIC_LATTICE_A, 0.05, 300.0, mi.BASE_SEED + 7)
+    n, K, box = s["n"], 32, list(s["box"])
+    d = {k: torch.from_numpy(s[k]).to(gpu.dev) for k in ("x", "y", "z", "vx", "vy", "vz")}
+    types = torch.from_numpy(s["types"]).to(gpu.dev)
+    pe = torch.zeros(n, dtype=torch.float64, device=gpu.dev)
+    f = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    W = torch.zeros((9, n), dtype=torch.float64, device=gpu.dev)
+    J = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    nl = md.md_neighbors_create(n, K)
+    md.md_build_neighbors(nl, n, d["x"], d["y"], d["z"], box, 3.5)
+
+    def call():
+        md.md_tersoff_multi_force(nl, n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], box, types,
+                                  mi.TERSOFF_SIC_ELEMENTS, mi.TERSOFF_SIC_CHI, md.MD_FP64, pe=pe, f=f, virial=W, heat=J)
+    for _ in range(max(3, warmup)):
+        call()
+    md.md_neighbors_status(nl)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+    gpu.barrier()
+    for a, b in ev:
+        gpu.flush_l2()
+        a.record(); call(); b.record()
+    torch.cuda.synchronize()
+    ms, = gpu_max([sum(a.elapsed_time(b) for a, b in ev)], gpu)
+    listed, in_range, triplets = md.md_pair_counts(nl)
+    md.md_neighbors_destroy(nl)
+    return {"workload": "3C-SiC 512000 atoms, multi-element Tersoff (Tersoff 1989 parameters)", "atoms": n,
+            "outputs": "pe, f, virial(9), heat", "calls": calls, "value": gpu.world * n * calls / (ms * 1e-3),
+            "unit": "atom-evals/s", "us_per_eval": 1e3 * ms / calls, "listed_per_atom": listed / n,
+            "in_range_per_atom": in_range / n, "ordered_triplets_per_atom": triplets / n}
+
+
 def summary(r):
     """The per-config entry of the line's `configs` object."""
     c = r["c"]
@@ -430,6 +466,7 @@ def main_ours(args):
             extra[mi.CONFIGS[idx]["name"] + ("_fp32" if fp32 else "")] = summary(q)
         extra["cfg1_tersoff_512_eval"] = measure_eval(gpu, md, 0, 200, args.warmup, fp64_peak, peaks)
         extra["cfg2_size_full_output_eval"] = measure_eval(gpu, md, 1, 20, args.warmup, fp64_peak, peaks)
+        extra["multi_element_sic_512k_eval"] = measure_multi_eval(gpu, md, 20, args.warmup, peaks)
     if gpu.rank != 0:
         gpu.close()
         return 0

@@ -104,6 +104,23 @@ int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double*
                      const md_tersoff_params* p, int precision,
                      double* pe, double* f, double* virial, double* heat, void* stream);
 
+/* Multi-element Tersoff ("systems with more than one type of atom"; reading A17 =
+ * Tersoff's multicomponent form): elem[t] are the per-element parameters, the pair (a,b) uses
+ * lambda, mu = arithmetic means, A, B, R, S = geometric means, and chi[a][b] (chi[a][a] = 1) multiplies the
+ * attractive term; g and b use c, d, h, beta, n of the CENTRAL atom.  types: DEVICE int32[n], values in
+ * 0..ntypes-1.  The list must have been built with r_list >= max S + skin.  n < 2^28.  Same outputs, layouts
+ * and error behaviour as md_tersoff_force; with ntypes = 1 it computes exactly that potential. */
+enum { MD_MAX_TYPES = 4 };
+typedef struct {
+    int ntypes;
+    md_tersoff_params elem[MD_MAX_TYPES];
+    double chi[MD_MAX_TYPES][MD_MAX_TYPES];
+} md_tersoff_multi_params;
+int md_tersoff_multi_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                           const double* vx, const double* vy, const double* vz, const double box[3],
+                           const int32_t* types, const md_tersoff_multi_params* p, int precision,
+                           double* pe, double* f, double* virial, double* heat, void* stream);
+
 /* Same for Stillinger-Weber; three-body energy is attributed to the central atom (reading A6). */
 int md_sw_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                 const double* vx, const double* vy, const double* vz, const double box[3],

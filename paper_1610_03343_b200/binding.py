@@ -32,6 +32,10 @@ class md_tersoff_params(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("A", "B", "lambda_", "mu", "beta", "n", "c", "d", "h", "R", "S")]
 
 
+class md_tersoff_multi_params(C.Structure):
+    _fields_ = [("ntypes", C.c_int), ("elem", md_tersoff_params * 4), ("chi", (C.c_double * 4) * 4)]
+
+
 class md_sw_params(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("epsilon", "sigma", "a", "lambda_", "gamma", "A", "B", "p", "q", "cos0")]
 
@@ -39,7 +43,8 @@ class md_sw_params(C.Structure):
 EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neighbors_status",
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
-           "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts")
+           "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts",
+           "md_tersoff_multi_force")
 
 _lib = None
 
@@ -164,6 +169,25 @@ def md_tersoff_force(nl, n, x, y, z, vx, vy, vz, box, params, precision=MD_FP64,
     _check(load().md_tersoff_force(nl._h, C.c_int64(n), _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy), _ptr(vz),
                                    _box(box), C.byref(p), C.c_int(precision), _ptr(pe), _ptr(f), _ptr(virial),
                                    _ptr(heat), _stream(stream)), "md_tersoff_force")
+
+
+def tersoff_multi_params(elements, chi) -> md_tersoff_multi_params:
+    p = md_tersoff_multi_params()
+    p.ntypes = len(elements)
+    for t, e in enumerate(elements):
+        p.elem[t] = tersoff_params(e)
+        for u in range(len(elements)):
+            p.chi[t][u] = float(chi[t][u])
+    return p
+
+
+def md_tersoff_multi_force(nl, n, x, y, z, vx, vy, vz, box, types, elements, chi, precision=MD_FP64,
+                           pe=None, f=None, virial=None, heat=None, stream=None):
+    p = tersoff_multi_params(elements, chi)
+    _check(load().md_tersoff_multi_force(nl._h, C.c_int64(n), _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy),
+                                         _ptr(vz), _box(box), _ptr(types), C.byref(p), C.c_int(precision),
+                                         _ptr(pe), _ptr(f), _ptr(virial), _ptr(heat), _stream(stream)),
+           "md_tersoff_multi_force")
 
 
 def md_sw_force(nl, n, x, y, z, vx, vy, vz, box, params, precision=MD_FP64,

@@ -232,6 +232,22 @@ int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double*
                              (cudaStream_t)stream);
 }
 
+int md_tersoff_multi_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                           const double* vx, const double* vy, const double* vz, const double box[3],
+                           const int32_t* types, const md_tersoff_multi_params* p, int precision,
+                           double* pe, double* f, double* virial, double* heat, void* stream) {
+    int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
+    if (rc != MD_OK) return rc;
+    if (p->ntypes < 1 || p->ntypes > MD_MAX_TYPES || n >= ((int64_t)1 << 28)) return MD_ERR_ARG;
+    if (p->ntypes > 1 && n > 0 && !types) return MD_ERR_ARG;
+    for (int t = 0; t < p->ntypes; ++t) {
+        const md_tersoff_params& e = p->elem[t];
+        if (!(e.S > e.R) || !(e.R > 0) || !(e.n > 0) || !(e.d != 0)) return MD_ERR_ARG;
+    }
+    return md_launch_tersoff_multi(nl, n, x, y, z, vx, vy, vz, box, types, p, precision, pe, f, virial, heat,
+                                   (cudaStream_t)stream);
+}
+
 int md_sw_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                 const double* vx, const double* vy, const double* vz, const double box[3],
                 const md_sw_params* p, int precision,

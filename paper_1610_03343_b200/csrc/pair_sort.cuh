@@ -78,10 +78,15 @@ struct SortScratch {
 // neighbours in flight: their list entries first, then their 3 U coordinates).  T is the arithmetic type of the
 // force kernel: in FP32 mode r_ij is formed in double, rounded to float, and the float d2 decides (reading
 // A10) -- for both ends.  Indices are 32-bit: n * max_neighbors <= 2e9 is checked at md_neighbors_create.
+// Force range per pair of elements (multi-element Tersoff): r2[ti * nt + tj] = S_ij^2.  nt = 1: one range.
+template <class T> struct RangeTab { int nt; T r2[16]; };
+
 template <class T, int U>
 __device__ __forceinline__ unsigned long long
 screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const double* __restrict__ y,
-           const double* __restrict__ z, const MinImage& mi, const int32_t* __restrict__ NL, T range2) {
+           const double* __restrict__ z, const MinImage& mi, const int32_t* __restrict__ NL,
+           const RangeTab<T>& rt, const int32_t* __restrict__ types) {
+    const int trow = types ? types[i] * rt.nt : 0;
     const double xi = x[i], yi = y[i], zi = z[i];
     unsigned long long mask = 0ull;
     for (int m0 = 0; m0 < nn; m0 += U) {
@@ -110,7 +115,10 @@ screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const d
         }
         unsigned bits = 0u;
 #pragma unroll
-        for (int u = 0; u < U; ++u) bits |= d2[u] < range2 ? 1u << u : 0u;
+        for (int u = 0; u < U; ++u) {
+            const T range2 = types ? rt.r2[trow + types[j[u]]] : rt.r2[0];
+            bits |= d2[u] < range2 ? 1u << u : 0u;
+        }
         const int left = nn - m0;                                // entries of this chunk that exist
         if (left < U) bits &= (1u << left) - 1u;
         mask |= (unsigned long long)bits << m0;
@@ -126,13 +134,13 @@ template <class T>
 __global__ void __launch_bounds__(256, 4)
 k_screen(unsigned n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-         T range2, unsigned long long* __restrict__ MASK) {
+         RangeTab<T> rt, const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const MinImage mi = make_min_image(Lx, Ly, Lz);
     int nn = NN[i];
     if (nn > 64) nn = 64;
-    MASK[i] = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, range2);
+    MASK[i] = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, rt, types);
 }
 
 // Dense record layout: the record of pair (i -> j) goes to the slot of row j that counts the in-range entries

@@ -25,6 +25,12 @@ struct TersoffDev {
     T minus_half_over_n;      // -1/(2n)
 };
 
+// Multi-element form (reading A17): per-pair mixed parameters and per-centre parameters.  NT = 1 is the
+// single-element potential (every index folds to 0 at compile time).
+template <class T> struct TsPair { T A, B, lambda, mu, R, w, chi; };     // w = pi / (S - R); B carries no chi
+template <class T> struct TsCenter { T beta, n, h, c2, d2, c2_over_d2, minus_half_over_n; };
+template <class T, int NT> struct TersoffTab { TsCenter<T> c[NT]; TsPair<T> p[NT * NT]; };
+
 constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom (generic path)
 
 // Generic path: any number of in-range neighbours up to TERSOFF_KC, per-thread arrays in local memory.
@@ -399,12 +405,13 @@ struct TersoffSortSmem {
     __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
-template <class T, class Rec, int BT, int PCA, int RMR, int MAXREG>
+template <class T, class Rec, int BT, int PCA, int RMR, int MAXREG, int NT>
 __global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
 k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                  const double* __restrict__ z, double Lx, double Ly, double Lz,
                  const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                 const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
+                 const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, NT> tab,
+                 const int32_t* __restrict__ types, const double* __restrict__ gtab,
                  Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                  double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                  int* __restrict__ status) {
@@ -425,7 +432,9 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
     const int64_t i = A0 + t;
     const int col = base + lane;                             // slot k of this thread: col + 32 k
 
-    if (Mw <= RMR) {
+    const int ti = NT > 1 ? types[i] : 0;
+    const TsCenter<T> pc = tab.c[ti];
+    if (NT == 1 && Mw <= RMR) {
         // every atom of this warp has at most RMR in-range neighbours (after the sort: most warps of a hot
         // crystal): compact them into register slots and run the straight-line register body
         int jd[RMR], rv[RMR];
@@ -494,19 +503,21 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
                 const T d2 = d2s[u];
                 const T ri = fm::rsqrt(d2);
                 const T r = d2 * ri;
+                const int tj = NT > 1 ? types[j[u]] : 0;
+                const TsPair<T> pp = tab.p[ti * NT + tj];    // mixed parameters of the pair (reading A17)
                 T c = T(1), cp = T(0);
-                if (r > p.R) {                               // f_C window R < r < S (reading A1)
+                if (r > pp.R) {                              // f_C window R < r < S (reading A1)
                     T sn, cs;
-                    fm::sincos_0_pi((r - p.R) * p.w, &sn, &cs);
+                    fm::sincos_0_pi((r - pp.R) * pp.w, &sn, &cs);
                     c = T(0.5) + T(0.5) * cs;
-                    cp = T(-0.5) * p.w * sn;
+                    cp = T(-0.5) * pp.w * sn;
                 }
                 const int q = col + 32 * (k0 + u);
                 s.ex[q] = tx * ri; s.ey[q] = ty * ri; s.ez[q] = tz * ri; s.rinv[q] = ri;
                 s.fc[q] = c; s.fcp[q] = cp;
-                s.fRD[q] = p.A * fm::exp(-p.lambda * r, tb);
-                s.fAh[q] = p.B * fm::exp(-p.mu * r, tb);
-                s.jj[q] = j[u];
+                s.fRD[q] = pp.A * fm::exp(-pp.lambda * r, tb);
+                s.fAh[q] = pp.chi * pp.B * fm::exp(-pp.mu * r, tb);         // chi_ij f_A: b_ij only ever multiplies it
+                s.jj[q] = j[u] | (tj << 28);                 // element of the neighbour in the top bits (n < 2^28)
             }
         }
     }
@@ -521,9 +532,9 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
         auto zterm = [&](int b) {
             const int cb = col + 32 * b;
             const T cs = ax * s.ex[cb] + ay * s.ey[cb] + az * s.ez[cb];
-            const T xx = p.h - cs;
+            const T xx = pc.h - cs;
             const T x2 = xx * xx;
-            zt += s.fc[cb] * (T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2));
+            zt += s.fc[cb] * (T(1) + pc.c2_over_d2 * x2 * fm::rcp(pc.d2 + x2));
         };
 #pragma unroll 2
         for (int b = 0; b < a; ++b) zterm(b);
@@ -531,14 +542,15 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
         for (int b = a + 1; b < M; ++b) zterm(b);
         T bo = T(1), bp = T(0);
         if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
-            const T tt = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);               // (beta zeta)^n
-            bo = fm::exp(p.minus_half_over_n * fm::log(T(1) + tt, tb), tb);         // Eq. (3)
+            const T tt = fm::exp(pc.n * fm::log(pc.beta * zt, tb), tb);             // (beta zeta)^n
+            bo = fm::exp(pc.minus_half_over_n * fm::log(T(1) + tt, tb), tb);        // Eq. (3)
             bp = T(-0.5) * bo * tt * fm::rcp(zt * (T(1) + tt));
         }
         const T c = s.fc[ca], cp = s.fcp[ca], fR = s.fRD[ca], fA = s.fAh[ca];
+        const TsPair<T> pp = tab.p[ti * NT + (NT > 1 ? (int)((unsigned)s.jj[ca] >> 28) : 0)];
         const T bfA = bo * fA;
         U += T(0.5) * c * (fR - bfA);                                                  // U_ia / 2
-        s.fRD[ca] = T(0.5) * (cp * (fR - bfA) + c * (p.mu * bfA - p.lambda * fR));     // D
+        s.fRD[ca] = T(0.5) * (cp * (fR - bfA) + c * (pp.mu * bfA - pp.lambda * fR));   // D
         s.fAh[ca] = T(-0.5) * c * fA * bp;                                             // h
     }
 
@@ -552,7 +564,7 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
         const int ca = col + 32 * a;
         const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
         const T ha = s.fAh[ca], fca = s.fc[ca], cpa = s.fcp[ca], ria = s.rinv[ca];
-        const int ja = s.jj[ca];
+        const int ja = s.jj[ca] & 0x0fffffff;
         const unsigned slot = ps::dense_slot(MASK[ja], (int)REV[(int64_t)m * n + i]);   // dense record layout
         T ce = s.fRD[ca];                                    // coefficient of e_a
         T sx = T(0), sy = T(0), sz = T(0);                   // sum of ta * e_b
@@ -560,13 +572,13 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
             const int cb = col + 32 * b;
             const T bx = s.ex[cb], by = s.ey[cb], bz = s.ez[cb];
             const T cs = ax * bx + ay * by + az * bz;
-            const T xx = p.h - cs;
+            const T xx = pc.h - cs;
             const T x2 = xx * xx;
-            const T q = fm::rcp(p.d2 + x2);
+            const T q = fm::rcp(pc.d2 + x2);
             const T hb = s.fAh[cb];
-            const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
+            const T gp = T(-2) * pc.c2 * xx * q * q;         // dg/dcos
             const T ta = (ha * s.fc[cb] + hb * fca) * gp * ria;
-            ce += hb * cpa * (T(1) + p.c2_over_d2 * x2 * q) - ta * cs;
+            ce += hb * cpa * (T(1) + pc.c2_over_d2 * x2 * q) - ta * cs;
             sx += ta * bx; sy += ta * by; sz += ta * bz;
         };
 #pragma unroll 2
@@ -592,16 +604,66 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
     }
 }
 
-template <class T, class Rec>
-int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
-           const double box[3], const md_tersoff_params* hp, double* pe, double* f, double* virial,
-           cudaStream_t s) {
+template <class T>
+TersoffDev<T> make_dev(const md_tersoff_params* hp) {
     TersoffDev<T> p;
     p.A = (T)hp->A; p.B = (T)hp->B; p.lambda = (T)hp->lambda; p.mu = (T)hp->mu; p.beta = (T)hp->beta;
     p.n = (T)hp->n; p.h = (T)hp->h; p.R = (T)hp->R; p.S2 = (T)(hp->S * hp->S);
     p.c2 = (T)(hp->c * hp->c); p.d2 = (T)(hp->d * hp->d); p.c2_over_d2 = (T)((hp->c * hp->c) / (hp->d * hp->d));
     p.w = (T)(3.14159265358979323846 / (hp->S - hp->R));
     p.minus_half_over_n = (T)(-0.5 / hp->n);
+    return p;
+}
+
+// Mixing rules of reading A17 (lambda, mu: arithmetic means; A, B, R, S: geometric means), computed in double.
+template <class T, int NT>
+void make_tab(const md_tersoff_multi_params* hp, TersoffTab<T, NT>* tab, ps::RangeTab<T>* rt) {
+    rt->nt = NT;
+    for (int a = 0; a < NT; ++a) {
+        const md_tersoff_params& e = hp->elem[a];
+        TsCenter<T>& c = tab->c[a];
+        c.beta = (T)e.beta; c.n = (T)e.n; c.h = (T)e.h; c.c2 = (T)(e.c * e.c); c.d2 = (T)(e.d * e.d);
+        c.c2_over_d2 = (T)((e.c * e.c) / (e.d * e.d)); c.minus_half_over_n = (T)(-0.5 / e.n);
+        for (int b = 0; b < NT; ++b) {
+            const md_tersoff_params& g = hp->elem[b];
+            const double R = sqrt(e.R * g.R), S = sqrt(e.S * g.S);
+            TsPair<T>& q = tab->p[a * NT + b];
+            q.A = (T)sqrt(e.A * g.A); q.B = (T)sqrt(e.B * g.B);
+            q.lambda = (T)(0.5 * (e.lambda + g.lambda)); q.mu = (T)(0.5 * (e.mu + g.mu));
+            q.R = (T)R; q.w = (T)(3.14159265358979323846 / (S - R)); q.chi = (T)hp->chi[a][b];
+            rt->r2[a * NT + b] = (T)(S * S);
+        }
+    }
+}
+
+template <class T, class Rec, int NT>
+int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                  const double box[3], const TersoffDev<T>& p, const md_tersoff_multi_params* mp,
+                  const int32_t* types, const double* gtab, double* pe, double* f, double* virial, cudaStream_t s) {
+    TersoffTab<T, NT> tab;
+    ps::RangeTab<T> rt;
+    make_tab<T, NT>(mp, &tab, &rt);
+    nl->launches[MD_KIND_PAIR] += 1;
+    ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2],
+                                                                 nl->NN, nl->NL, rt, NT > 1 ? types : nullptr, nl->MASK);
+    nl->q_dense = 1;
+    constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
+    using Sm = TersoffSortSmem<T, BT, PCA>;
+    auto kern = k_tersoff_sorted<T, Rec, BT, PCA, 4, 168, NT>;
+    const int rca = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
+    if (rca != MD_OK) return rca;
+    kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
+        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types, gtab, (Rec*)nl->Q, nl->MASK,
+        pe, f, virial, nl->d_status);
+    MD_CUDA_TRY(cudaGetLastError());
+    return MD_OK;
+}
+
+template <class T, class Rec>
+int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+           const double box[3], const md_tersoff_params* hp, double* pe, double* f, double* virial,
+           cudaStream_t s) {
+    const TersoffDev<T> p = make_dev<T>(hp);
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
@@ -617,20 +679,9 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     const int rcs = md_list_row_stats(nl, &max_row, &long_rows, 0);
     if (rcs != MD_OK) return rcs;
     if ((int64_t)long_rows * 256 > n) {
-        nl->launches[MD_KIND_PAIR] += 1;
-        ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2],
-                                                                     nl->NN, nl->NL, p.S2, nl->MASK);
-        nl->q_dense = 1;
-        constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
-        using Sm = TersoffSortSmem<T, BT, PCA>;
-        auto kern = k_tersoff_sorted<T, Rec, BT, PCA, 4, 168>;
-        const int rca = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
-        if (rca != MD_OK) return rca;
-        kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
-            n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
-            pe, f, virial, nl->d_status);
-        MD_CUDA_TRY(cudaGetLastError());
-        return MD_OK;
+        md_tersoff_multi_params one;
+        one.ntypes = 1; one.elem[0] = *hp; one.chi[0][0] = 1.0;
+        return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, &one, nullptr, gtab, pe, f, virial, s);
     }
     nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
     MD_TERSOFF_LAUNCH(4, 128, 168);
@@ -639,7 +690,34 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     return MD_OK;
 }
 
+template <class T, class Rec>
+int launch_multi(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                 const double box[3], const int32_t* types, const md_tersoff_multi_params* mp, double* pe,
+                 double* f, double* virial, cudaStream_t s) {
+    const TersoffDev<T> p = make_dev<T>(&mp->elem[0]);       // used by the single-element register body only
+    ProfScope prof(nl, MD_KIND_PAIR, 1, s);
+    const double* gtab = md_math_tables();
+    if (!gtab) return MD_ERR_ALLOC;
+    switch (mp->ntypes) {
+        case 1: return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, mp, nullptr, gtab, pe, f, virial, s);
+        case 2: return launch_sorted<T, Rec, 2>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
+        case 3: return launch_sorted<T, Rec, 3>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
+        default: return launch_sorted<T, Rec, 4>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
+    }
+}
+
 }  // namespace
+
+int md_launch_tersoff_multi(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                            const double* vx, const double* vy, const double* vz, const double box[3],
+                            const int32_t* types, const md_tersoff_multi_params* p, int precision, double* pe,
+                            double* f, double* virial, double* heat, cudaStream_t s) {
+    if (n == 0) return MD_OK;
+    int rc = precision == MD_FP32 ? launch_multi<float, float4>(nl, n, x, y, z, box, types, p, pe, f, virial, s)
+                                  : launch_multi<double, PairRec64>(nl, n, x, y, z, box, types, p, pe, f, virial, s);
+    if (rc != MD_OK) return rc;
+    return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, nullptr, s);
+}
 
 int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                       const double* vx, const double* vy, const double* vz, const double box[3],

