@@ -421,6 +421,36 @@ def measure_multi_eval(gpu, md, calls, warmup, peaks):
             "in_range_per_atom": in_range / n, "ordered_triplets_per_atom": triplets / n}
 
 
+def measure_literal_ab(gpu, md, cfg_index, calls, warmup):
+    """the paper's literal Algorithm 3 + 2 (md_tersoff_force_literal) beside the stored-P design
+    (md_tersoff_force), forces only, same list, per-call event pairs, L2 flushed before every call."""
+    torch = gpu.torch
+    c = mi.make_config(cfg_index)
+    n, K, box = c["n"], c["max_neighbors"], list(c["box"])
+    d = {k: torch.from_numpy(c[k]).to(gpu.dev) for k in ("x", "y", "z", "vx", "vy", "vz")}
+    f = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+    nl = md.md_neighbors_create(n, K)
+    md.md_build_neighbors(nl, n, d["x"], d["y"], d["z"], box, c["r_list"])
+    out = {"workload": c["name"], "atoms": n, "outputs": "f"}
+    for name, fn in (("stored_P", md.md_tersoff_force), ("literal_alg3_alg2", md.md_tersoff_force_literal)):
+        def call():
+            fn(nl, n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], box, c["params"], md.MD_FP64, f=f)
+        for _ in range(max(3, warmup)):
+            call()
+        md.md_neighbors_status(nl)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(calls)]
+        gpu.barrier()
+        for a, b in ev:
+            gpu.flush_l2()
+            a.record(); call(); b.record()
+        torch.cuda.synchronize()
+        ms, = gpu_max([sum(a.elapsed_time(b) for a, b in ev)], gpu)
+        out[name] = {"us_per_eval": 1e3 * ms / calls, "atom_evals_per_s": gpu.world * n * calls / (ms * 1e-3)}
+    md.md_neighbors_destroy(nl)
+    out["literal_over_stored"] = out["literal_alg3_alg2"]["us_per_eval"] / out["stored_P"]["us_per_eval"]
+    return out
+
+
 def summary(r):
     """The per-config entry of the line's `configs` object."""
     c = r["c"]
@@ -467,6 +497,8 @@ def main_ours(args):
         extra["cfg1_tersoff_512_eval"] = measure_eval(gpu, md, 0, 200, args.warmup, fp64_peak, peaks)
         extra["cfg2_size_full_output_eval"] = measure_eval(gpu, md, 1, 20, args.warmup, fp64_peak, peaks)
         extra["multi_element_sic_512k_eval"] = measure_multi_eval(gpu, md, 20, args.warmup, peaks)
+        extra["literal_vs_stored_P_cfg2"] = measure_literal_ab(gpu, md, 1, 20, args.warmup)
+        extra["literal_vs_stored_P_cfg4"] = measure_literal_ab(gpu, md, 3, 5, args.warmup)
     if gpu.rank != 0:
         gpu.close()
         return 0

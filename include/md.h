@@ -104,6 +104,15 @@ int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double*
                      const md_tersoff_params* p, int precision,
                      double* pe, double* f, double* virial, double* heat, void* stream);
 
+/* The paper's literal two-kernel scheme as an A/B against the stored-P design: Algorithm 3
+ * stores b_ij and db_ij/dzeta_ij per listed pair (16 bytes), Algorithm 2
+ * recomputes dU_j/dr_ji inside thread i and writes every per-atom output once; no pair records, no gather
+ * kernel.  Same arguments, outputs and tolerances as md_tersoff_force. */
+int md_tersoff_force_literal(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                             const double* vx, const double* vy, const double* vz, const double box[3],
+                             const md_tersoff_params* p, int precision,
+                             double* pe, double* f, double* virial, double* heat, void* stream);
+
 /* Multi-element Tersoff ("systems with more than one type of atom"; reading A17 =
  * Tersoff's multicomponent form): elem[t] are the per-element parameters, the pair (a,b) uses
  * lambda, mu = arithmetic means, A, B, R, S = geometric means, and chi[a][b] (chi[a][a] = 1) multiplies the

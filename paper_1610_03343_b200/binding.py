@@ -44,7 +44,7 @@ EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neig
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
            "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts",
-           "md_tersoff_multi_force")
+           "md_tersoff_multi_force", "md_tersoff_force_literal")
 
 _lib = None
 
@@ -169,6 +169,15 @@ def md_tersoff_force(nl, n, x, y, z, vx, vy, vz, box, params, precision=MD_FP64,
     _check(load().md_tersoff_force(nl._h, C.c_int64(n), _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy), _ptr(vz),
                                    _box(box), C.byref(p), C.c_int(precision), _ptr(pe), _ptr(f), _ptr(virial),
                                    _ptr(heat), _stream(stream)), "md_tersoff_force")
+
+
+def md_tersoff_force_literal(nl, n, x, y, z, vx, vy, vz, box, params, precision=MD_FP64,
+                             pe=None, f=None, virial=None, heat=None, stream=None):
+    """The paper's literal Algorithm 3 + Algorithm 2 (A/B against the stored-P design)."""
+    p = tersoff_params(params)
+    _check(load().md_tersoff_force_literal(nl._h, C.c_int64(n), _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy),
+                                           _ptr(vz), _box(box), C.byref(p), C.c_int(precision), _ptr(pe), _ptr(f),
+                                           _ptr(virial), _ptr(heat), _stream(stream)), "md_tersoff_force_literal")
 
 
 def tersoff_multi_params(elements, chi) -> md_tersoff_multi_params:

@@ -232,6 +232,17 @@ int md_tersoff_force(md_neighbors* nl, int64_t n, const double* x, const double*
                              (cudaStream_t)stream);
 }
 
+int md_tersoff_force_literal(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                             const double* vx, const double* vy, const double* vz, const double box[3],
+                             const md_tersoff_params* p, int precision,
+                             double* pe, double* f, double* virial, double* heat, void* stream) {
+    int rc = check_force_args(nl, n, x, y, z, vx, vy, vz, box, p, precision, heat);
+    if (rc != MD_OK) return rc;
+    if (!(p->S > p->R) || !(p->R > 0) || !(p->n > 0) || !(p->d != 0)) return MD_ERR_ARG;
+    return md_launch_tersoff_literal(nl, n, x, y, z, vx, vy, vz, box, p, precision, pe, f, virial, heat,
+                                     (cudaStream_t)stream);
+}
+
 int md_tersoff_multi_force(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                            const double* vx, const double* vy, const double* vz, const double box[3],
                            const int32_t* types, const md_tersoff_multi_params* p, int precision,

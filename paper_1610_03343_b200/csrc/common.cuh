@@ -117,6 +117,10 @@ int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double
                       const double* vx, const double* vy, const double* vz, const double box[3],
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
                       double* heat, const VVFuse* vv, cudaStream_t s);
+int md_launch_tersoff_literal(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
+                              const double* vx, const double* vy, const double* vz, const double box[3],
+                              const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
+                              double* heat, cudaStream_t s);
 int md_launch_tersoff_multi(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                             const double* vx, const double* vy, const double* vz, const double box[3],
                             const int32_t* types, const md_tersoff_multi_params* p, int precision, double* pe,
