@@ -154,6 +154,20 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
                double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
                int first_step, int nsteps, int rebuild_every, double r_list, void* stream);
 
+/* NPT by weak coupling: Berendsen thermostat and barostat, the paper's benchmark ensemble (
+ * SURVEY 8(f-3); reading A18).  Each step is a velocity-Verlet step (as md_nve_run) followed by
+ *   T = 2 KE / (3 n kB),  P = (2 KE + tr sum_i W_i) / (3 V)      with W_i from the force call (Eq. 29)
+ *   v *= sqrt(1 + (dt/tau_T)(T0/T - 1));   x, box *= (1 - beta (dt/tau_P)(P0 - P))^(1/3)
+ * T0 in K, tau in fs, P0 in eV/A^3 (1 eV/A^3 = 160.21766 GPa), beta (compressibility) in A^3/eV.
+ * box: HOST double[3], read and UPDATED.  T_trace, P_trace: HOST [nsteps] (may be NULL), the values measured
+ * before each step's scaling.  The call reads two scalars back per step, so it synchronises `stream`. */
+typedef struct { double T0, tau_T, P0, tau_P, beta; } md_berendsen_params;
+int md_npt_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+               double* x, double* y, double* z, double* vx, double* vy, double* vz,
+               double* f, int f_valid, double box[3], double mass_amu, double dt_fs,
+               int first_step, int nsteps, int rebuild_every, double r_list,
+               const md_berendsen_params* b, double* T_trace, double* P_trace, void* stream);
+
 /* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
  * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
  * synchronises.  Device buffers are owned by the handle.  Returns the latched device status (as

@@ -186,6 +186,27 @@ def evaluate_multi(elements, chi, types, x, y, z, box, NN, NL, v=None, precision
     return out
 
 
+def npt_run(potential, params, state, nsteps, dt, rebuild_every, r_list, K, berendsen, f=None):
+    """Berendsen NPT (reading A18); `state` as in nve_run, its box is updated in place.
+    berendsen = dict(T0, tau_T, P0, tau_P, beta) in K, fs, eV/A^3, fs, A^3/eV.
+    Returns dict(f, T_trace, P_trace) with the values measured before each step's scaling."""
+    n = state["x"].size
+    par = pack_params(potential, params)
+    f_valid = 0 if f is None else 1
+    f = np.zeros((3, n)) if f is None else np.ascontiguousarray(f, dtype=np.float64)
+    Tt, Pt = np.zeros(max(nsteps, 1)), np.zeros(max(nsteps, 1))
+    b = berendsen
+    rc = lib().oracle_npt_run(C.c_int(pot_id(potential)), _p(par), C.c_int64(n), _p(state["x"]), _p(state["y"]),
+                              _p(state["z"]), _p(state["vx"]), _p(state["vy"]), _p(state["vz"]), _p(state["box"]),
+                              C.c_double(state["mass"]), C.c_double(dt), C.c_int(nsteps), C.c_int(rebuild_every),
+                              C.c_double(r_list), C.c_int(K), _p(f), C.c_int(f_valid), C.c_double(b["T0"]),
+                              C.c_double(b["tau_T"]), C.c_double(b["P0"]), C.c_double(b["tau_P"]),
+                              C.c_double(b["beta"]), _p(Tt), _p(Pt))
+    if rc != 0:
+        raise RuntimeError(f"oracle_npt_run failed rc={rc}")
+    return {"f": f, "T_trace": Tt[:nsteps], "P_trace": Pt[:nsteps]}
+
+
 def atom_energy_multi(elements, chi, ti, tj, rvecs) -> float:
     r = np.ascontiguousarray(rvecs, dtype=np.float64)
     rx, ry, rz = (np.ascontiguousarray(r[:, a]) for a in range(3))

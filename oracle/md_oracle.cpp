@@ -738,4 +738,56 @@ int oracle_nve_run(int pot, const double* par, int64_t n, double* x, double* y, 
     return 0;
 }
 
+// NPT by weak coupling (Berendsen thermostat and barostat: the paper's benchmark ensemble, PAPER.md:355;
+// DESIGN.md reading A18).  One step = velocity-Verlet step, then
+//   T = 2 KE / (3 N kB),  P = (2 KE + tr sum_i W_i) / (3 V)        (W = sum r_i (x) F_i, Eq. 17)
+//   v *= lambda,  lambda = sqrt(1 + (dt/tau_T)(T0/T - 1))
+//   x, box *= mu, mu = (1 - beta (dt/tau_P)(P0 - P))^(1/3)
+// P in eV/A^3, beta in A^3/eV.  T_trace, P_trace [nsteps] receive the values measured BEFORE the scaling.
+int oracle_npt_run(int pot, const double* par, int64_t n, double* x, double* y, double* z,
+                   double* vx, double* vy, double* vz, double* box, double mass, double dt,
+                   int nsteps, int rebuild_every, double r_list, int K, double* f, int f_valid,
+                   double T0, double tau_T, double P0, double tau_P, double beta,
+                   double* T_trace, double* P_trace) {
+    const double KB = 8.617333262e-5;
+    std::vector<int32_t> NN(n), NL((size_t)n * K);
+    std::vector<double> pe(n), W((size_t)9 * n);
+    auto forces = [&]() {
+        return evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
+                                pe.data(), f, nullptr, W.data(), nullptr, nullptr, 0, n);
+    };
+    if (!f_valid) {
+        if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
+        int rc = forces();
+        if (rc) return rc;
+    }
+    for (int s = 0; s < nsteps; ++s) {
+        vv_kick_drift(n, x, y, z, vx, vy, vz, f, mass, dt, box);
+        if (s % rebuild_every == 0 || !f_valid)
+            if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
+        f_valid = 1;
+        int rc = forces();
+        if (rc) return rc;
+        vv_kick(n, vx, vy, vz, f, mass, dt);
+        long double ke2 = 0, trw = 0;                                      // 2 KE and tr W
+        for (int64_t i = 0; i < n; ++i) {
+            ke2 += (long double)(vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i]);
+            trw += (long double)(W[0 * n + i] + W[4 * n + i] + W[8 * n + i]);
+        }
+        ke2 *= mass / KAPPA_ACC;
+        const double V = box[0] * box[1] * box[2];
+        const double T = (double)ke2 / (3.0 * n * KB), P = (double)(ke2 + trw) / (3.0 * V);
+        if (T_trace) T_trace[s] = T;
+        if (P_trace) P_trace[s] = P;
+        const double lam = T > 0 ? std::sqrt(1.0 + dt / tau_T * (T0 / T - 1.0)) : 1.0;
+        const double mu = std::cbrt(1.0 - beta * dt / tau_P * (P0 - P));
+        for (int64_t i = 0; i < n; ++i) {
+            vx[i] *= lam; vy[i] *= lam; vz[i] *= lam;
+            x[i] *= mu; y[i] *= mu; z[i] *= mu;
+        }
+        for (int a = 0; a < 3; ++a) box[a] *= mu;
+    }
+    return 0;
+}
+
 }  // extern "C"

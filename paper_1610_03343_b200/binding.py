@@ -44,7 +44,7 @@ EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neig
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
            "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts",
-           "md_tersoff_multi_force", "md_tersoff_force_literal")
+           "md_tersoff_multi_force", "md_tersoff_force_literal", "md_npt_run")
 
 _lib = None
 
@@ -236,6 +236,29 @@ def md_nve_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, pe, bo
                              C.c_int(1 if f_valid else 0), _ptr(pe), _box(box), C.c_double(mass_amu),
                              C.c_double(dt_fs), C.c_int(first_step), C.c_int(nsteps), C.c_int(rebuild_every),
                              C.c_double(r_list), _stream(stream)), "md_nve_run")
+
+
+class md_berendsen_params(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("T0", "tau_T", "P0", "tau_P", "beta")]
+
+
+def md_npt_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, box, mass_amu, dt_fs, nsteps,
+               rebuild_every, r_list, berendsen, precision=MD_FP64, stream=None, first_step=0):
+    """Berendsen NPT.  `box` is a list of 3 floats and is UPDATED in place; returns (T_trace, P_trace) lists."""
+    import ctypes
+    pid, p = _pot(potential, params)
+    b = md_berendsen_params(berendsen["T0"], berendsen["tau_T"], berendsen["P0"], berendsen["tau_P"], berendsen["beta"])
+    cbox = _box(box)
+    Tt = (ctypes.c_double * max(1, nsteps))()
+    Pt = (ctypes.c_double * max(1, nsteps))()
+    _check(load().md_npt_run(nl._h, C.c_int(pid), C.byref(p), C.c_int(precision), C.c_int64(n), _ptr(x), _ptr(y),
+                             _ptr(z), _ptr(vx), _ptr(vy), _ptr(vz), _ptr(f), C.c_int(1 if f_valid else 0), cbox,
+                             C.c_double(mass_amu), C.c_double(dt_fs), C.c_int(first_step), C.c_int(nsteps),
+                             C.c_int(rebuild_every), C.c_double(r_list), C.byref(b), Tt, Pt, _stream(stream)),
+           "md_npt_run")
+    for a in range(3):
+        box[a] = cbox[a]
+    return list(Tt)[:nsteps], list(Pt)[:nsteps]
 
 
 def md_nve_run_host(nl, potential, params, n, x, y, z, vx, vy, vz, f, pe, box, mass_amu, dt_fs,

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI declared in include/md.h: argument checks, handle life cycle, and the host-side
 // composition of the kernels.  No arithmetic of the method lives here.
+#include <cmath>
 #include <mutex>
 #include <new>
 #include <set>
@@ -14,7 +15,8 @@ bool valid_box(const double box[3]) { return box && box[0] > 0 && box[1] > 0 && 
 void free_all(md_neighbors* nl) {
     cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
-    cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e);
+    cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e); cudaFree(nl->npt_w); cudaFree(nl->npt_part);
+    if (nl->h_npt) cudaFreeHost(nl->h_npt);
     if (nl->h_maxrow) cudaFreeHost(nl->h_maxrow);
     if (nl->ev_list) cudaEventDestroy(nl->ev_list);
     if (nl->ev_pool) for (cudaEvent_t e : *nl->ev_pool) cudaEventDestroy(e);
@@ -318,6 +320,62 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
         vv.mode = last ? 1 : 2;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  last ? pe : nullptr, f, nullptr, nullptr, &vv, s)) != MD_OK) return rc;
+    }
+    return MD_OK;
+}
+
+int md_npt_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+               double* x, double* y, double* z, double* vx, double* vy, double* vz,
+               double* f, int f_valid, double box[3], double mass_amu, double dt_fs,
+               int first_step, int nsteps, int rebuild_every, double r_list,
+               const md_berendsen_params* b, double* T_trace, double* P_trace, void* stream) {
+    if (!nl || !params || !b || n < 1 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1 ||
+        first_step < 0)
+        return MD_ERR_ARG;
+    if (potential != MD_TERSOFF && potential != MD_SW) return MD_ERR_ARG;
+    if (precision != MD_FP64 && precision != MD_FP32) return MD_ERR_ARG;
+    if (!(mass_amu > 0) || !(r_list > 0) || !(b->tau_T > 0) || !(b->tau_P > 0)) return MD_ERR_ARG;
+    if (!x || !y || !z || !vx || !vy || !vz || !f) return MD_ERR_ARG;
+    for (int a = 0; a < 3; ++a)
+        if ((int)(box[a] / r_list) < 3) return MD_ERR_BOX_TOO_SMALL;
+    if (f_valid && nsteps > 0 && first_step % rebuild_every != 0 && nl->n != n) return MD_ERR_NO_LIST;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (nl->npt_cap < n || !nl->npt_w) {
+        MD_CUDA_TRY(cudaStreamSynchronize(s));
+        cudaFree(nl->npt_w); nl->npt_w = nullptr; nl->npt_cap = 0;
+        if (cudaMalloc(&nl->npt_w, sizeof(double) * 9 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+        nl->npt_cap = n;
+    }
+    if (!nl->npt_part) {
+        if (cudaMalloc(&nl->npt_part, sizeof(double) * md_npt_scratch_doubles()) != cudaSuccess ||
+            cudaMallocHost(&nl->h_npt, 2 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+    }
+    int rc;
+    double* W = nl->npt_w;
+    if (!f_valid) {
+        if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
+    }
+    for (int step = first_step; step < first_step + nsteps; ++step) {
+        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if (step % rebuild_every == 0)
+            if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if (nl->n != n) return MD_ERR_NO_LIST;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
+        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        double sums[2];
+        if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, sums, s)) != MD_OK) return rc;
+        const double ke2 = sums[0] * mass_amu / MD_KAPPA;                 // 2 KE
+        const double V = box[0] * box[1] * box[2];
+        const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + sums[1]) / (3.0 * V);
+        if (T_trace) T_trace[step - first_step] = T;
+        if (P_trace) P_trace[step - first_step] = P;
+        const double lam = T > 0 ? sqrt(1.0 + dt_fs / b->tau_T * (b->T0 / T - 1.0)) : 1.0;
+        const double mu = cbrt(1.0 - b->beta * dt_fs / b->tau_P * (b->P0 - P));
+        if ((rc = md_launch_npt_scale(nl, n, x, y, z, vx, vy, vz, lam, mu, s)) != MD_OK) return rc;
+        for (int a = 0; a < 3; ++a) box[a] *= mu;
     }
     return MD_OK;
 }

@@ -64,6 +64,8 @@ struct md_neighbors {
     std::vector<int>* ev_kind;                         // kind of each recorded pair
     size_t ev_used;                                    // events handed out since the last read
     double ms_acc[MD_N_KINDS];
+    // Berendsen NPT (md_npt_run): per-atom virial [9][n], reduction scratch, pinned landing zone
+    double* npt_w; int64_t npt_cap; double* npt_part; double* h_npt;
     // e2e device state (md_nve_run_host)
     double* e2e;            // [13][n] x,y,z,vx,vy,vz,f[3],pe + spare
     int64_t e2e_cap;
@@ -78,6 +80,7 @@ __device__ __forceinline__ double md_min_image(double d, double L, double halfL)
 
 // velocity-Verlet pieces shared by integrate.cu and the fused gather kernel
 constexpr double MD_KAPPA = 9.648533215665e-3;   // (A/fs^2) per (eV/A/amu)
+constexpr double MD_KB = 8.617333262e-5;         // Boltzmann constant, eV/K
 __device__ __forceinline__ double md_wrap(double c, double L) {
     c -= L * floor(c / L);
     return (c >= L || c < 0.0) ? 0.0 : c;        // reading A8
@@ -136,4 +139,9 @@ int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, d
                  const double* f, double mass, double dt, const double box[3], cudaStream_t s);
 const double* md_math_tables();   // device tables of fastmath.cuh for the current device (nullptr on failure)
 int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);
+int md_launch_npt_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
+                       const double* W, double out[2], cudaStream_t s);
+int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
+                        double* vz, double lam, double mu, cudaStream_t s);
+int md_npt_scratch_doubles();
 int md_launch_pair_counts(md_neighbors* nl, int64_t out[3], cudaStream_t s);

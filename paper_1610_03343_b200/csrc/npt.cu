@@ -1,0 +1,63 @@
+// npt.cu -- Berendsen weak coupling (thermostat + barostat), the paper's benchmark ensemble (PAPER.md:355:
+// "NPT ensemble ... Berendsen"), reading A18.  Consumes sum_i W_i.
+//   k_npt_partial / k_npt_final  sum_i |v_i|^2 and sum_i (W_xx + W_yy + W_zz): fixed grid, fixed order, no
+//                                atomics -> the same bits run to run
+//   k_npt_scale                  v *= lambda;  x *= mu
+#include "common.cuh"
+
+namespace {
+constexpr int RED_BLOCKS = 296, RED_BT = 256;
+
+__global__ void __launch_bounds__(RED_BT)
+k_npt_partial(int64_t n, const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+              const double* __restrict__ W, double* __restrict__ part) {
+    __shared__ double s_a[RED_BT / 32], s_b[RED_BT / 32];
+    double a = 0.0, b = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * RED_BT + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_BT) {
+        a += vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i];
+        b += W[i] + W[4 * n + i] + W[8 * n + i];
+    }
+    for (int d = 16; d > 0; d >>= 1) { a += __shfl_down_sync(0xffffffffu, a, d); b += __shfl_down_sync(0xffffffffu, b, d); }
+    if ((threadIdx.x & 31) == 0) { s_a[threadIdx.x >> 5] = a; s_b[threadIdx.x >> 5] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double ta = 0.0, tb = 0.0;
+        for (int w = 0; w < RED_BT / 32; ++w) { ta += s_a[w]; tb += s_b[w]; }
+        part[2 * blockIdx.x] = ta; part[2 * blockIdx.x + 1] = tb;
+    }
+}
+__global__ void k_npt_final(const double* __restrict__ part, double* __restrict__ out) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double ta = 0.0, tb = 0.0;
+    for (int k = 0; k < RED_BLOCKS; ++k) { ta += part[2 * k]; tb += part[2 * k + 1]; }
+    out[0] = ta; out[1] = tb;
+}
+__global__ void k_npt_scale(int64_t n, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
+                            double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
+                            double lam, double mu) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    vx[i] *= lam; vy[i] *= lam; vz[i] *= lam;
+    x[i] *= mu; y[i] *= mu; z[i] *= mu;
+}
+}  // namespace
+
+// sum v^2 and tr sum W -> HOST out[2]; synchronises the stream
+int md_launch_npt_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
+                       const double* W, double out[2], cudaStream_t s) {
+    ProfScope prof(nl, MD_KIND_INTEGRATE, 2, s);
+    k_npt_partial<<<RED_BLOCKS, RED_BT, 0, s>>>(n, vx, vy, vz, W, nl->npt_part);
+    k_npt_final<<<1, 32, 0, s>>>(nl->npt_part, nl->npt_part + 2 * RED_BLOCKS);
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_npt, nl->npt_part + 2 * RED_BLOCKS, 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaStreamSynchronize(s));
+    out[0] = nl->h_npt[0]; out[1] = nl->h_npt[1];
+    return MD_OK;
+}
+int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
+                        double* vz, double lam, double mu, cudaStream_t s) {
+    ProfScope prof(nl, MD_KIND_INTEGRATE, 1, s);
+    k_npt_scale<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, x, y, z, vx, vy, vz, lam, mu);
+    MD_CUDA_TRY(cudaGetLastError());
+    return MD_OK;
+}
+int md_npt_scratch_doubles() { return 2 * RED_BLOCKS + 2; }

@@ -186,3 +186,54 @@ def test_threaded_evaluation_equals_single_thread():
         pe, f = oracle.evaluate_threads(pot, par, s["x"], s["y"], s["z"], s["box"], NN, NL, 3)
         assert (pe == ref["pe"]).all()
         assert np.abs(f - ref["f"]).max() <= 1e-13 * np.abs(ref["f"]).max()
+
+
+# ---------------------------------------------------------------- Berendsen NPT (reading A18)
+BER = dict(T0=300.0, tau_T=100.0, P0=0.0, tau_P=1000.0, beta=1.0 / 0.61)     # beta ~ 1/B of Si (98 GPa = 0.61 eV/A^3)
+
+
+def dilute_gas(n=64, L=200.0, T=900.0, seed=3):
+    """Atoms further apart than any cut-off for the whole run: no forces, P = N kB T / V exactly."""
+    rng = np.random.default_rng(seed)
+    g = np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing="ij"), -1).reshape(-1, 3)[:n] * 40.0 + 20.0
+    sv = math.sqrt(mi.KB_EV_PER_K * T / mi.SI_MASS_AMU * mi.KAPPA)
+    v = rng.normal(size=(n, 3)) * sv
+    return {"x": g[:, 0].copy(), "y": g[:, 1].copy(), "z": g[:, 2].copy(), "vx": v[:, 0].copy(),
+            "vy": v[:, 1].copy(), "vz": v[:, 2].copy(), "box": np.array([L, L, L]), "mass": mi.SI_MASS_AMU, "n": n}
+
+
+def test_berendsen_ideal_gas_closed_forms():
+    """Without forces the weak-coupling recursions close: T_{k+1} = T_k + (dt/tau_T)(T0 - T_k), and with
+    P = N kB T / V the volume obeys V_{k+1} = V_k (1 - beta dt/tau_P (P0 - P_k)).  Pins thermostat, barostat,
+    the temperature and pressure definitions and their units."""
+    s = dilute_gas()
+    n, dt, steps = s["n"], 1.0, 40
+    v2 = (s["vx"] ** 2 + s["vy"] ** 2 + s["vz"] ** 2).sum()
+    T = s["mass"] * v2 / mi.KAPPA / (3 * n * mi.KB_EV_PER_K)
+    V = float(np.prod(s["box"]))
+    ber = dict(BER, P0=2e-7, tau_P=50.0, beta=1000.0)
+    r = oracle.npt_run("tersoff", mi.TERSOFF_SI_C, s, steps, dt, 10, 3.5, 16, ber)
+    for k in range(steps):
+        P = n * mi.KB_EV_PER_K * T / V
+        assert abs(r["T_trace"][k] - T) <= 1e-12 * T, k
+        assert abs(r["P_trace"][k] - P) <= 1e-12 * P, k
+        T, V = T + dt / ber["tau_T"] * (ber["T0"] - T), V * (1.0 - ber["beta"] * dt / ber["tau_P"] * (ber["P0"] - P))
+        # positions and box are scaled AFTER the measurement, so the scaled velocities' T follows next step
+    assert abs(float(np.prod(s["box"])) - V) <= 1e-12 * V
+
+
+def test_berendsen_crystal_relaxes_to_zero_pressure_lattice_constant():
+    """Physics pin: a cold Tersoff crystal started 1 % expanded contracts towards the zero-pressure lattice
+    constant of the potential (5.432 A, tests/golden).  With beta = 1/B (B = 97.8 GPa = 0.6104 eV/A^3, the
+    bulk modulus pinned in test_oracle_pins) weak coupling makes the pressure decay as exp(-t/tau_P)."""
+    x, y, z, L = mi.diamond_lattice(2, 5.432 * 1.01)
+    n = x.size
+    s = {"x": x, "y": y, "z": z, "vx": np.zeros(n), "vy": np.zeros(n), "vz": np.zeros(n),
+         "box": np.array([L, L, L]), "mass": mi.SI_MASS_AMU, "n": n}
+    ber = dict(T0=1.0, tau_T=50.0, P0=0.0, tau_P=200.0, beta=1.0 / 0.6104)
+    r = oracle.npt_run("tersoff", mi.TERSOFF_SI_C, s, 1000, 1.0, 10, 3.5, 16, ber)
+    P = r["P_trace"]
+    assert P[0] < 0                                              # expanded crystal: tensile
+    assert 0.30 <= P[200] / P[0] <= 0.45                         # e^-1 = 0.37 (B softens a little under tension)
+    assert abs(P[-1]) < 0.02 * abs(P[0])                         # e^-5
+    assert abs(s["box"][0] / 2 - 5.432) < 0.001
