@@ -266,23 +266,43 @@ k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __res
             j[u] = NL[(int64_t)m * n + i];
             if (CHECK && (unsigned)j[u] >= (unsigned long long)n) { atomicOr(&status[0], MD_DEV_NO_REVERSE); j[u] = (int)i; }
         }
+        // The first four entries of every partner row are read unconditionally (16 independent loads: for
+        // crystal rows that is the whole answer after two dependent levels); the position is the number of
+        // entries smaller than i, and only if all four are smaller does a binary search of [4, NN[j]) follow.
+        int nj[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { lo[u] = 0; hi[u] = min(NN[j[u]], K); }
-        // lower bound of i in row j; rows have at most 64 entries: 7 halvings reach lo == hi
+        for (int u = 0; u < 4; ++u) nj[u] = min(NN[j[u]], K);
+        int head[4][4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) head[u][q] = NL[(int64_t)(q < K ? q : 0) * n + j[u]];
+        bool live = false;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            int c = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) c += (q < nj[u] && head[u][q] < (int)i) ? 1 : 0;
+            lo[u] = c;
+            hi[u] = c == 4 ? nj[u] : c;                          // c < 4: found (lo == hi); else search [4, nj)
+            live = live || lo[u] < hi[u];
+        }
+        if (__any_sync(__activemask(), live)) {
 #pragma unroll 1
-        for (int it = 0; it < 7; ++it) {
-            int v[4], mid[4];
-            bool live = false;
+            for (int it = 0; it < 7; ++it) {                     // rows have at most 64 entries
+                int v[4], mid[4];
+                bool more = false;
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                mid[u] = (lo[u] + hi[u]) >> 1;
-                live = live || lo[u] < hi[u];
-                v[u] = lo[u] < hi[u] ? NL[(int64_t)mid[u] * n + j[u]] : 0;
+                for (int u = 0; u < 4; ++u) {
+                    mid[u] = (lo[u] + hi[u]) >> 1;
+                    more = more || lo[u] < hi[u];
+                    v[u] = lo[u] < hi[u] ? NL[(int64_t)mid[u] * n + j[u]] : 0;
+                }
+                if (!__any_sync(__activemask(), more)) break;
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (lo[u] < hi[u]) { if (v[u] < (int)i) lo[u] = mid[u] + 1; else hi[u] = mid[u]; }
             }
-            if (!__any_sync(__activemask(), live)) break;
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (lo[u] < hi[u]) { if (v[u] < (int)i) lo[u] = mid[u] + 1; else hi[u] = mid[u]; }
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
