@@ -168,6 +168,18 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
                int first_step, int nsteps, int rebuild_every, double r_list,
                const md_berendsen_params* b, double* T_trace, double* P_trace, void* stream);
 
+/* Green-Kubo workload (the application of the paper's Ref. [27]): NVE steps as
+ * md_nve_run (unfused), and after every `sample_every`-th step the total heat current of that state:
+ *   J_pot = sum_i J_i (Eq. 30)      J_kin = sum_i (m v_i^2 / 2 + U_i) v_i   (convective part)
+ * in eV A/fs.  J_pot, J_kin: HOST [nsteps / sample_every][3] (either may be NULL).  Reads six scalars back per
+ * sample, so it synchronises `stream`.  The autocorrelation and its integral are the caller's
+ * (paper_1610_03343_b200.green_kubo). */
+int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+                    double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                    double* f, int f_valid, const double box[3], double mass_amu, double dt_fs,
+                    int first_step, int nsteps, int rebuild_every, double r_list, int sample_every,
+                    double* J_pot, double* J_kin, void* stream);
+
 /* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
  * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
  * synchronises.  Device buffers are owned by the handle.  Returns the latched device status (as

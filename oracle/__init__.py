@@ -186,6 +186,25 @@ def evaluate_multi(elements, chi, types, x, y, z, box, NN, NL, v=None, precision
     return out
 
 
+def nve_heat_run(potential, params, state, nsteps, dt, rebuild_every, r_list, K, sample_every, f=None):
+    """NVE with the total heat current sampled every `sample_every` steps (Green-Kubo workload).
+    Returns dict(f, J_pot[ns][3], J_kin[ns][3])."""
+    n = state["x"].size
+    par = pack_params(potential, params)
+    f_valid = 0 if f is None else 1
+    f = np.zeros((3, n)) if f is None else np.ascontiguousarray(f, dtype=np.float64)
+    ns = nsteps // sample_every
+    Jp, Jk = np.zeros((max(ns, 1), 3)), np.zeros((max(ns, 1), 3))
+    rc = lib().oracle_nve_heat_run(C.c_int(pot_id(potential)), _p(par), C.c_int64(n), _p(state["x"]), _p(state["y"]),
+                                   _p(state["z"]), _p(state["vx"]), _p(state["vy"]), _p(state["vz"]),
+                                   _p(_f64(state["box"])), C.c_double(state["mass"]), C.c_double(dt), C.c_int(nsteps),
+                                   C.c_int(rebuild_every), C.c_double(r_list), C.c_int(K), _p(f), C.c_int(f_valid),
+                                   C.c_int(sample_every), _p(Jp), _p(Jk))
+    if rc != 0:
+        raise RuntimeError(f"oracle_nve_heat_run failed rc={rc}")
+    return {"f": f, "J_pot": Jp[:ns], "J_kin": Jk[:ns]}
+
+
 def npt_run(potential, params, state, nsteps, dt, rebuild_every, r_list, K, berendsen, f=None):
     """Berendsen NPT (reading A18); `state` as in nve_run, its box is updated in place.
     berendsen = dict(T0, tau_T, P0, tau_P, beta) in K, fs, eV/A^3, fs, A^3/eV.

@@ -738,6 +738,62 @@ int oracle_nve_run(int pot, const double* par, int64_t n, double* x, double* y, 
     return 0;
 }
 
+// NVE with the total heat current sampled every `sample_every` steps (the Green-Kubo workload of the paper's
+// Ref. [27]).  After the step's second half-kick:
+//   J_pot = sum_i J_i,  J_i = sum_j r_ij (dU_j/dr_ji . v_i)                 (Eq. 30 / Eq. 25)
+//   J_kin = sum_i (1/2 m v_i^2 + U_i) v_i                                    (convective part, reading A12)
+// J_pot[ns][3], J_kin[ns][3] (either may be NULL), ns = number of steps s with (s + 1) % sample_every == 0.
+int oracle_nve_heat_run(int pot, const double* par, int64_t n, double* x, double* y, double* z,
+                        double* vx, double* vy, double* vz, const double* box, double mass, double dt,
+                        int nsteps, int rebuild_every, double r_list, int K, double* f, int f_valid,
+                        int sample_every, double* J_pot, double* J_kin) {
+    std::vector<int32_t> NN(n), NL((size_t)n * K);
+    std::vector<double> pe(n), J((size_t)3 * n);
+    if (!f_valid) {
+        if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
+        int rc = evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
+                                  pe.data(), f, nullptr, nullptr, nullptr, nullptr, 0, n);
+        if (rc) return rc;
+    }
+    int ns = 0;
+    for (int s = 0; s < nsteps; ++s) {
+        vv_kick_drift(n, x, y, z, vx, vy, vz, f, mass, dt, box);
+        if (s % rebuild_every == 0 || !f_valid)
+            if (neighbours_cell(n, x, y, z, box, r_list, K, NN.data(), NL.data()) < 0) return -1;
+        f_valid = 1;
+        const bool sample = (s + 1) % sample_every == 0;
+        int rc;
+        if (!sample) {
+            rc = evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
+                                  pe.data(), f, nullptr, nullptr, nullptr, nullptr, 0, n);
+            if (rc) return rc;
+            vv_kick(n, vx, vy, vz, f, mass, dt);
+            continue;
+        }
+        // Eq. (30) uses v_i of the state the forces belong to: kick first with the new forces, then evaluate J
+        rc = evaluate<double>(pot, par, n, x, y, z, nullptr, nullptr, nullptr, box, NN.data(), NL.data(), K,
+                              pe.data(), f, nullptr, nullptr, nullptr, nullptr, 0, n);
+        if (rc) return rc;
+        vv_kick(n, vx, vy, vz, f, mass, dt);
+        std::vector<double> f2((size_t)3 * n);
+        rc = evaluate<double>(pot, par, n, x, y, z, vx, vy, vz, box, NN.data(), NL.data(), K,
+                              pe.data(), f2.data(), nullptr, nullptr, J.data(), nullptr, 0, n);
+        if (rc) return rc;
+        long double jp[3] = {0, 0, 0}, jk[3] = {0, 0, 0};
+        for (int64_t i = 0; i < n; ++i) {
+            const double e = 0.5 * mass / KAPPA_ACC * (vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i]) + pe[i];
+            jp[0] += J[i]; jp[1] += J[n + i]; jp[2] += J[2 * n + i];
+            jk[0] += e * vx[i]; jk[1] += e * vy[i]; jk[2] += e * vz[i];
+        }
+        for (int a = 0; a < 3; ++a) {
+            if (J_pot) J_pot[3 * ns + a] = (double)jp[a];
+            if (J_kin) J_kin[3 * ns + a] = (double)jk[a];
+        }
+        ++ns;
+    }
+    return 0;
+}
+
 // NPT by weak coupling (Berendsen thermostat and barostat: the paper's benchmark ensemble, PAPER.md:355;
 // DESIGN.md reading A18).  One step = velocity-Verlet step, then
 //   T = 2 KE / (3 N kB),  P = (2 KE + tr sum_i W_i) / (3 V)        (W = sum r_i (x) F_i, Eq. 17)

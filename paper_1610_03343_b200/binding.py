@@ -44,7 +44,7 @@ EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neig
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
            "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts",
-           "md_tersoff_multi_force", "md_tersoff_force_literal", "md_npt_run")
+           "md_tersoff_multi_force", "md_tersoff_force_literal", "md_npt_run", "md_nve_heat_run")
 
 _lib = None
 
@@ -259,6 +259,23 @@ def md_npt_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, box, m
     for a in range(3):
         box[a] = cbox[a]
     return list(Tt)[:nsteps], list(Pt)[:nsteps]
+
+
+def md_nve_heat_run(nl, potential, params, n, x, y, z, vx, vy, vz, f, f_valid, box, mass_amu, dt_fs, nsteps,
+                    rebuild_every, r_list, sample_every, precision=MD_FP64, stream=None, first_step=0):
+    """NVE with the total heat current sampled every `sample_every` steps.  Returns (J_pot, J_kin) as lists of
+    [Jx, Jy, Jz] per sample (eV A/fs)."""
+    pid, p = _pot(potential, params)
+    ns = nsteps // sample_every
+    Jp = (C.c_double * max(1, 3 * ns))()
+    Jk = (C.c_double * max(1, 3 * ns))()
+    _check(load().md_nve_heat_run(nl._h, C.c_int(pid), C.byref(p), C.c_int(precision), C.c_int64(n), _ptr(x), _ptr(y),
+                                  _ptr(z), _ptr(vx), _ptr(vy), _ptr(vz), _ptr(f), C.c_int(1 if f_valid else 0),
+                                  _box(box), C.c_double(mass_amu), C.c_double(dt_fs), C.c_int(first_step),
+                                  C.c_int(nsteps), C.c_int(rebuild_every), C.c_double(r_list), C.c_int(sample_every),
+                                  Jp, Jk, _stream(stream)), "md_nve_heat_run")
+    return ([[Jp[3 * k + a] for a in range(3)] for k in range(ns)],
+            [[Jk[3 * k + a] for a in range(3)] for k in range(ns)])
 
 
 def md_nve_run_host(nl, potential, params, n, x, y, z, vx, vy, vz, f, pe, box, mass_amu, dt_fs,

@@ -348,7 +348,7 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
     }
     if (!nl->npt_part) {
         if (cudaMalloc(&nl->npt_part, sizeof(double) * md_npt_scratch_doubles()) != cudaSuccess ||
-            cudaMallocHost(&nl->h_npt, 2 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+            cudaMallocHost(&nl->h_npt, 6 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
     }
     int rc;
     double* W = nl->npt_w;
@@ -376,6 +376,67 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
         const double mu = cbrt(1.0 - b->beta * dt_fs / b->tau_P * (b->P0 - P));
         if ((rc = md_launch_npt_scale(nl, n, x, y, z, vx, vy, vz, lam, mu, s)) != MD_OK) return rc;
         for (int a = 0; a < 3; ++a) box[a] *= mu;
+    }
+    return MD_OK;
+}
+
+int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+                    double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                    double* f, int f_valid, const double box[3], double mass_amu, double dt_fs,
+                    int first_step, int nsteps, int rebuild_every, double r_list, int sample_every,
+                    double* J_pot, double* J_kin, void* stream) {
+    if (!nl || !params || n < 1 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1 ||
+        first_step < 0 || sample_every < 1)
+        return MD_ERR_ARG;
+    if (potential != MD_TERSOFF && potential != MD_SW) return MD_ERR_ARG;
+    if (precision != MD_FP64 && precision != MD_FP32) return MD_ERR_ARG;
+    if (!(mass_amu > 0) || !(r_list > 0)) return MD_ERR_ARG;
+    if (!x || !y || !z || !vx || !vy || !vz || !f) return MD_ERR_ARG;
+    for (int a = 0; a < 3; ++a)
+        if ((int)(box[a] / r_list) < 3) return MD_ERR_BOX_TOO_SMALL;
+    if (f_valid && nsteps > 0 && first_step % rebuild_every != 0 && nl->n != n) return MD_ERR_NO_LIST;
+    cudaStream_t s = (cudaStream_t)stream;
+    // scratch: per-atom heat current [3][n] and energy [n] live in the NPT virial buffer ([9][n])
+    if (nl->npt_cap < n || !nl->npt_w) {
+        MD_CUDA_TRY(cudaStreamSynchronize(s));
+        cudaFree(nl->npt_w); nl->npt_w = nullptr; nl->npt_cap = 0;
+        if (cudaMalloc(&nl->npt_w, sizeof(double) * 9 * (size_t)n) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+        nl->npt_cap = n;
+    }
+    if (!nl->npt_part) {
+        if (cudaMalloc(&nl->npt_part, sizeof(double) * md_npt_scratch_doubles()) != cudaSuccess ||
+            cudaMallocHost(&nl->h_npt, 6 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+    }
+    double* J = nl->npt_w;
+    double* pe = nl->npt_w + 3 * n;
+    int rc, ns = 0;
+    if (!f_valid) {
+        if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 nullptr, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
+    }
+    for (int step = first_step; step < first_step + nsteps; ++step) {
+        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if (step % rebuild_every == 0)
+            if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
+        if (nl->n != n) return MD_ERR_NO_LIST;
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 nullptr, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
+        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if ((step - first_step + 1) % sample_every != 0) continue;
+        // Eq. (30) with the velocities of this state: the pair records are still valid, one more gather
+        if ((rc = md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, nullptr, nullptr, J, nullptr, s)) != MD_OK)
+            return rc;
+        // U_i of this state for the convective part (a second pair pass: the fused NVE path never stores it)
+        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
+                                 pe, nullptr, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
+        double out[6];
+        if ((rc = md_launch_heat_sums(nl, n, vx, vy, vz, pe, J, mass_amu, out, s)) != MD_OK) return rc;
+        for (int a = 0; a < 3; ++a) {
+            if (J_pot) J_pot[3 * ns + a] = out[a];
+            if (J_kin) J_kin[3 * ns + a] = out[3 + a];
+        }
+        ++ns;
     }
     return MD_OK;
 }

@@ -143,5 +143,7 @@ int md_launch_npt_sums(md_neighbors* nl, int64_t n, const double* vx, const doub
                        const double* W, double out[2], cudaStream_t s);
 int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
                         double* vz, double lam, double mu, cudaStream_t s);
+int md_launch_heat_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
+                        const double* pe, const double* J, double mass, double out[6], cudaStream_t s);
 int md_npt_scratch_doubles();
 int md_launch_pair_counts(md_neighbors* nl, int64_t out[3], cudaStream_t s);

@@ -60,4 +60,49 @@ int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, doubl
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
 }
-int md_npt_scratch_doubles() { return 2 * RED_BLOCKS + 2; }
+
+// ---- Green-Kubo workload: J_pot = sum_i J_i and J_kin = sum_i (m v_i^2 / 2 + U_i) v_i, same fixed-order scheme
+namespace {
+__global__ void __launch_bounds__(RED_BT)
+k_heat_partial(int64_t n, const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+               const double* __restrict__ pe, const double* __restrict__ J, double half_m, double* __restrict__ part) {
+    __shared__ double s_v[6][RED_BT / 32];
+    double a[6] = {0, 0, 0, 0, 0, 0};
+    for (int64_t i = (int64_t)blockIdx.x * RED_BT + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_BT) {
+        const double ux = vx[i], uy = vy[i], uz = vz[i];
+        const double e = half_m * (ux * ux + uy * uy + uz * uz) + pe[i];
+        a[0] += J[i]; a[1] += J[n + i]; a[2] += J[2 * n + i];
+        a[3] += e * ux; a[4] += e * uy; a[5] += e * uz;
+    }
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+        for (int d = 16; d > 0; d >>= 1) a[q] += __shfl_down_sync(0xffffffffu, a[q], d);
+        if ((threadIdx.x & 31) == 0) s_v[q][threadIdx.x >> 5] = a[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double t = 0.0;
+        for (int w = 0; w < RED_BT / 32; ++w) t += s_v[threadIdx.x][w];
+        part[6 * blockIdx.x + threadIdx.x] = t;
+    }
+}
+__global__ void k_heat_final(const double* __restrict__ part, double* __restrict__ out) {
+    if (blockIdx.x != 0 || threadIdx.x >= 6) return;
+    double t = 0.0;
+    for (int k = 0; k < RED_BLOCKS; ++k) t += part[6 * k + threadIdx.x];
+    out[threadIdx.x] = t;
+}
+}  // namespace
+
+// HOST out[6] = J_pot (3), J_kin (3); synchronises the stream
+int md_launch_heat_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
+                        const double* pe, const double* J, double mass, double out[6], cudaStream_t s) {
+    ProfScope prof(nl, MD_KIND_INTEGRATE, 2, s);
+    k_heat_partial<<<RED_BLOCKS, RED_BT, 0, s>>>(n, vx, vy, vz, pe, J, 0.5 * mass / MD_KAPPA, nl->npt_part);
+    k_heat_final<<<1, 32, 0, s>>>(nl->npt_part, nl->npt_part + 6 * RED_BLOCKS);
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_npt, nl->npt_part + 6 * RED_BLOCKS, 6 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaStreamSynchronize(s));
+    for (int q = 0; q < 6; ++q) out[q] = nl->h_npt[q];
+    return MD_OK;
+}
+int md_npt_scratch_doubles() { return 6 * RED_BLOCKS + 6; }

@@ -237,3 +237,37 @@ def test_berendsen_crystal_relaxes_to_zero_pressure_lattice_constant():
     assert 0.30 <= P[200] / P[0] <= 0.45                         # e^-1 = 0.37 (B softens a little under tension)
     assert abs(P[-1]) < 0.02 * abs(P[0])                         # e^-5
     assert abs(s["box"][0] / 2 - 5.432) < 0.001
+
+
+# ---------------------------------------------------------------- Green-Kubo heat-current time series
+def test_heat_current_series_is_the_energy_moment_rate():
+    """Pins oracle_nve_heat_run against the identity P12 uses for a single evaluation, now along a trajectory:
+    on a free (vacuum-padded) cluster d/dt sum_i r_i E_i = J_kin + J_pot, so the series' time integral over a
+    window equals the change of the energy moment R = sum_i r_i E_i (trapezoid rule, error O(dt^2))."""
+    x, y, z, L = mi.diamond_lattice(2)
+    rng = np.random.default_rng(8)
+    n = x.size
+    box = np.array([60.0, 60.0, 60.0])
+    s = {"x": x + 20 + rng.normal(size=n) * 0.05, "y": y + 20 + rng.normal(size=n) * 0.05,
+         "z": z + 20 + rng.normal(size=n) * 0.05, "box": box, "mass": mi.SI_MASS_AMU, "n": n}
+    v = rng.normal(size=(n, 3)) * 3e-3
+    v -= v.mean(axis=0)
+    s["vx"], s["vy"], s["vz"] = v[:, 0].copy(), v[:, 1].copy(), v[:, 2].copy()
+
+    def moment(st):
+        NN, NL = oracle.neighbors(st["x"], st["y"], st["z"], box, 3.5, 16)
+        pe = oracle.evaluate("tersoff", mi.TERSOFF_SI_C, st["x"], st["y"], st["z"], box, NN, NL, want=("pe",))["pe"]
+        e = 0.5 * st["mass"] / mi.KAPPA * (st["vx"] ** 2 + st["vy"] ** 2 + st["vz"] ** 2) + pe
+        return np.array([(st[k] * e).sum() for k in "xyz"])
+    errs = []
+    for dt in (0.4, 0.2):
+        st = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in s.items()}
+        r0 = oracle.nve_heat_run("tersoff", mi.TERSOFF_SI_C, st, 1, dt, 10, 3.5, 16, 1)     # J at t = dt
+        R0 = moment(st)
+        nst = int(round(8.0 / dt))
+        r = oracle.nve_heat_run("tersoff", mi.TERSOFF_SI_C, st, nst, dt, 10, 3.5, 16, 1, f=r0["f"])
+        R1 = moment(st)
+        Jt = np.vstack([r0["J_pot"] + r0["J_kin"], r["J_pot"] + r["J_kin"]])                 # t = dt .. dt (1 + nst)
+        integral = dt * (Jt[0] / 2 + Jt[1:-1].sum(axis=0) + Jt[-1] / 2)
+        errs.append(np.abs(integral - (R1 - R0)).max() / np.abs(R1 - R0).max())
+    assert errs[0] < 2e-2 and 3.3 <= errs[0] / errs[1] <= 5.0, errs      # trapezoid + Verlet: O(dt^2)
