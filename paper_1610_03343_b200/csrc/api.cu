@@ -13,7 +13,7 @@ namespace {
 bool valid_box(const double box[3]) { return box && box[0] > 0 && box[1] > 0 && box[2] > 0; }
 
 void free_all(md_neighbors* nl) {
-    cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK);
+    cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK); cudaFree(nl->bin_list); cudaFree(nl->bin_count);
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e); cudaFree(nl->npt_w); cudaFree(nl->npt_part);
     if (nl->h_npt) cudaFreeHost(nl->h_npt);
@@ -149,6 +149,8 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->REV, n * K) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->Q, n * K * sizeof(PairRec64)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->MASK, n * sizeof(unsigned long long)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->bin_list, 3 * n * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->bin_count, 4 * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->cell_of, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->rank_in_cell, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;

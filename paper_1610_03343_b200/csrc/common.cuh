@@ -37,6 +37,8 @@ struct md_neighbors {
     // per-pair records, pushed layout: Q[m*n + i] = P_{j i}, j = NL[m][i]
     void* Q;                // K*n*32 bytes
     unsigned long long* MASK;  // [n] bit m set <=> slot m is inside the force range
+    int32_t* bin_list;      // [3][n] atom indices by in-range-count bin (pair_sort.cuh, Bins), written by k_screen
+    int32_t* bin_count;     // [3]
     int q_dense;            // layout of the records the last pair kernel wrote: 1 = slot counts in-range entries
                             // (sorted kernels, MASK known beforehand), 0 = slot is the list position
     // cell structures

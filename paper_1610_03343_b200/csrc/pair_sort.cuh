@@ -70,6 +70,7 @@ template <int BT>
 struct SortScratch {
     unsigned long long mask[BT];     // in-range bits over the list row of atom t (tile order)
     unsigned short perm[BT];         // perm[rank] = t
+    int atom[BT];                    // atom index of tile entry t (-1: none)
     int cnt[BT / 32][MBINS + 3];     // per warp: atoms with M == b; then exclusive offsets (padded: 36 ints)
     int wmax[BT / 32];               // per warp (after the sort): largest M
 };
@@ -130,17 +131,43 @@ screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const d
 // loads (list entry -> coordinates), so it runs with small CTAs and few registers at full occupancy instead
 // of inside the pair kernel (whose shared-memory pool holds it to 12-16 warps per SM), and it makes every
 // MASK known before any pair record is written, which is what the dense record layout needs (dense_slot).
+// Bins of atoms by their number M of in-range neighbours: bin 0: M <= b0, bin 1: b0 < M <= b1, bin 2: M > b1.
+// The screen appends every atom to the index list of its bin (one atomic per warp and bin; the order inside a
+// list is whatever the warps' atomics make it, which is harmless: what is computed for an atom does not depend
+// on which thread computes it).  Each bin then gets a kernel specialised for its M.
+struct Bins {
+    int b0, b1;
+    int32_t* list;      // [3][n]
+    int32_t* count;     // [3], zeroed before the screen
+};
+
 template <class T>
 __global__ void __launch_bounds__(256, 4)
 k_screen(unsigned n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-         RangeTab<T> rt, const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK) {
+         RangeTab<T> rt, const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK, Bins bins) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const MinImage mi = make_min_image(Lx, Ly, Lz);
-    int nn = NN[i];
-    if (nn > 64) nn = 64;
-    MASK[i] = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, rt, types);
+    int bin = -1;
+    if (i < n) {
+        const MinImage mi = make_min_image(Lx, Ly, Lz);
+        int nn = NN[i];
+        if (nn > 64) nn = 64;
+        const unsigned long long mask = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, rt, types);
+        MASK[i] = mask;
+        const int M = __popcll(mask);
+        bin = M <= bins.b0 ? 0 : (M <= bins.b1 ? 1 : 2);
+    }
+    if (!bins.list) return;
+    const unsigned lane = threadIdx.x & 31;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const unsigned v = __ballot_sync(0xffffffffu, bin == b);
+        if (!v) continue;
+        int base = 0;
+        if (lane == (unsigned)(__ffs(v) - 1)) base = atomicAdd(&bins.count[b], __popc(v));
+        base = __shfl_sync(0xffffffffu, base, __ffs(v) - 1);
+        if (bin == b) bins.list[(size_t)b * n + base + __popc(v & ((1u << lane) - 1u))] = (int)i;
+    }
 }
 
 // Dense record layout: the record of pair (i -> j) goes to the slot of row j that counts the in-range entries

@@ -285,7 +285,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     ps::RangeTab<T> rt;
     rt.nt = 1; rt.r2[0] = p.rc2;
     ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2], nl->NN,
-                                                                 nl->NL, rt, nullptr, nl->MASK);
+                                                                 nl->NL, rt, nullptr, nl->MASK, ps::Bins{0, 0, nullptr, nullptr});
     nl->q_dense = 1;
     constexpr int BT = 128, PCA = MD_SW_POOL_PER_ATOM;
     using Sm = SWSmem<T, BT, PCA>;

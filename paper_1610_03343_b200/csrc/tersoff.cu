@@ -386,6 +386,56 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
     tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
 }
 
+// Register path for a bin of atoms with at most MR in-range neighbours (pair_sort.cuh, Bins): thread t of CTA
+// `cta` takes atom list[cta * BT + t], compacts its in-range list entries (bits of MASK) into MR register slots
+// and runs the straight-line body.  Records go to the dense slots (every MASK is known: k_screen ran before).
+// The math tables are staged by the calling kernel.
+template <class T, class Rec, int MR, int BT>
+__device__ __forceinline__ void
+tersoff_binned_cta(int64_t cta, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                   const double* __restrict__ z, double Lx, double Ly, double Lz,
+                   const int32_t* __restrict__ NL, const uint8_t* __restrict__ REV,
+                   const int32_t* __restrict__ list, const int32_t* __restrict__ count, const TersoffDev<T>& p,
+                   const fm::Tab& tb, Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                   double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial) {
+    const int64_t cnt = *count;
+    const int64_t t0 = cta * BT + threadIdx.x;
+    if (t0 >= cnt) return;                                   // no barrier follows
+    const int64_t i = list[t0];
+    unsigned long long run = MASK[i];
+    const int M = min(__popcll(run), MR);
+    int jd[MR], rv[MR];
+#pragma unroll
+    for (int k = 0; k < MR; ++k) {
+        const int m = run ? __ffsll((long long)run) - 1 : 0;
+        const unsigned q = (unsigned)m * (unsigned)n + (unsigned)i;
+        jd[k] = run ? NL[q] : (int)i;                        // an empty slot points at the atom itself
+        rv[k] = (int)REV[q];
+        run &= run - 1;
+    }
+    const double xi = x[i], yi = y[i], zi = z[i];
+    double qx[MR], qy[MR], qz[MR];
+    unsigned long long mj[MR];
+#pragma unroll
+    for (int k = 0; k < MR; ++k) { qx[k] = x[jd[k]]; qy[k] = y[jd[k]]; qz[k] = z[jd[k]]; mj[k] = MASK[jd[k]]; }
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
+    bool far = false;
+#pragma unroll
+    for (int k = 0; k < MR; ++k) {
+        qx[k] -= xi; qy[k] -= yi; qz[k] -= zi;
+        far = far || mi.far(ps::in_range_d2((T)qx[k], (T)qy[k], (T)qz[k]));
+        rv[k] = (int)ps::dense_slot(mj[k], rv[k]);           // dense record layout
+    }
+    if (__any_sync(__activemask(), far)) {
+#pragma unroll
+        for (int k = 0; k < MR; ++k) mi.wrap(qx[k], qy[k], qz[k]);
+    }
+    T ex[MR], ey[MR], ez[MR];
+#pragma unroll
+    for (int k = 0; k < MR; ++k) { ex[k] = (T)qx[k]; ey[k] = (T)qy[k]; ez[k] = (T)qz[k]; }
+    tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, (1u << M) - 1u, jd, rv, p, tb, Q, pe, f, virial);
+}
+
 // ---------------------------------------------------------------------------------------------------
 // Loop kernel for list rows of any length (config 5: 4-9 listed, 3-6 in range; rows longer than 4 are what
 // the register kernel cannot hold).  One thread per atom; the CTA first screens its atoms and reassigns them
@@ -395,7 +445,7 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
 //   pass 2  per slot a: zeta_ia over the other slots, b, b', U_ia/2; D_a and h_a replace f_R, f_A
 //   pass 3  per slot a: P_ia (T5), pushed to Q[rev(i,a)*n + j_a]; own halves in registers
 // Ordered pairs (a,b) and (b,a) are both visited: nothing here relies on g_ijk = g_ikj.
-// Warps whose atoms all have at most RMR in-range neighbours leave the loops for the register body above.
+// With one element it only sees the atoms of the long-row bin (k_tersoff_binned takes the others).
 template <class T, int BT, int PCA>
 struct TersoffSortSmem {
     ps::SortScratch<BT> ss;
@@ -405,68 +455,41 @@ struct TersoffSortSmem {
     __align__(16) double tab[fm::TAB_DOUBLES];
 };
 
-template <class T, class Rec, int BT, int PCA, int RMR, int MAXREG, int NT>
-__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
-k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
-                 const double* __restrict__ z, double Lx, double Ly, double Lz,
-                 const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                 const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, NT> tab,
-                 const int32_t* __restrict__ types, const double* __restrict__ gtab,
-                 Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-                 double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-                 int* __restrict__ status) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
+// CTA `cta` of `nctas` CTAs that share the tiles; tables staged (and the block synchronised) by the caller.
+template <class T, class Rec, int BT, int PCA, int NT>
+__device__ __forceinline__ void
+tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, const fm::Tab& tb, int64_t n,
+                    const double* __restrict__ x, const double* __restrict__ y,
+                    const double* __restrict__ z, double Lx, double Ly, double Lz,
+                    const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                    const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const TersoffTab<T, NT>& tab,
+                    const int32_t* __restrict__ types, const int32_t* __restrict__ list,
+                    const int32_t* __restrict__ count,
+                    Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                    double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+                    int* __restrict__ status) {
     const int tid = threadIdx.x, lane = tid & 31;
-    const int64_t A0 = (int64_t)blockIdx.x * BT;
-    const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
-    // in-range masks of the tile (k_screen wrote them), tile order
-    const unsigned long long mask0 = A0 + tid < n ? MASK[A0 + tid] : 0ull;
+    // a tile: BT consecutive atoms, or BT consecutive entries of a bin's index list (pair_sort.cuh, Bins); the
+    // grid strides over the tiles (a bin may hold few atoms: a grid sized for "all atoms" would mostly launch
+    // CTAs that exit at once, 25 us of nothing at 512 000 atoms)
+    const int64_t cnt = list ? (int64_t)*count : n;
+    for (int64_t A0 = cta * BT; A0 < cnt; A0 += nctas * BT) {
+    __syncthreads();                                         // the previous tile is done with the scratch
+    const int64_t a0 = A0 + tid < cnt ? (list ? (int64_t)list[A0 + tid] : A0 + tid) : -1;
+    s.ss.atom[tid] = (int)a0;
+    const unsigned long long mask0 = a0 >= 0 ? MASK[a0] : 0ull;   // in-range mask (k_screen wrote it)
     int t, base, Mw;
     unsigned long long mk;
     ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
     const int M = min(__popcll(mk), Mw);
-    if (A0 + t >= n) return;                                 // tile tail (M = 0); no barrier follows
-    const int64_t i = A0 + t;
+    const int64_t i = s.ss.atom[t];
+    if (i < 0) continue;                                     // tile tail (M = 0); the loop's barrier is reached by all
     const int col = base + lane;                             // slot k of this thread: col + 32 k
 
     const int ti = NT > 1 ? types[i] : 0;
     const TsCenter<T> pc = tab.c[ti];
-    if (NT == 1 && Mw <= RMR) {
-        // every atom of this warp has at most RMR in-range neighbours (after the sort: most warps of a hot
-        // crystal): compact them into register slots and run the straight-line register body
-        int jd[RMR], rv[RMR];
-        unsigned long long run = mk;
-#pragma unroll
-        for (int k = 0; k < RMR; ++k) {
-            const int m = run ? __ffsll((long long)run) - 1 : 0;
-            jd[k] = run ? NL[(int64_t)m * n + i] : (int)i;   // an empty slot points at the atom itself
-            rv[k] = (int)REV[(int64_t)m * n + i];
-            run &= run - 1;
-        }
-#pragma unroll
-        for (int k = 0; k < RMR; ++k) rv[k] = (int)ps::dense_slot(MASK[jd[k]], rv[k]);   // dense record layout
-        const double xi = x[i], yi = y[i], zi = z[i];
-        double qx[RMR], qy[RMR], qz[RMR];
-        bool far = false;
-#pragma unroll
-        for (int k = 0; k < RMR; ++k) {
-            qx[k] = x[jd[k]] - xi; qy[k] = y[jd[k]] - yi; qz[k] = z[jd[k]] - zi;
-            far = far || mi.far(ps::in_range_d2((T)qx[k], (T)qy[k], (T)qz[k]));
-        }
-        if (__any_sync(__activemask(), far)) {
-#pragma unroll
-            for (int k = 0; k < RMR; ++k) mi.wrap(qx[k], qy[k], qz[k]);
-        }
-        T ex[RMR], ey[RMR], ez[RMR];
-#pragma unroll
-        for (int k = 0; k < RMR; ++k) { ex[k] = (T)qx[k]; ey[k] = (T)qy[k]; ez[k] = (T)qz[k]; }
-        tersoff_reg_body<T, Rec, RMR>(i, n, ex, ey, ez, (1u << M) - 1u, jd, rv, p, tb, Q, pe, f, virial);
-        return;
-    }
-
     // pass 1
     {
         const double xi = x[i], yi = y[i], zi = z[i];
@@ -602,6 +625,54 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
 #pragma unroll
         for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
     }
+    }   // tiles
+}
+
+// The loop code on all atoms (several elements) or on one bin's list.
+template <class T, class Rec, int BT, int PCA, int NT>
+__global__ void __launch_bounds__(BT)
+k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
+                 const double* __restrict__ z, double Lx, double Ly, double Lz,
+                 const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                 const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, NT> tab,
+                 const int32_t* __restrict__ types, const int32_t* __restrict__ list,
+                 const int32_t* __restrict__ count, const double* __restrict__ gtab,
+                 Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                 double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+                 int* __restrict__ status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);
+    __syncthreads();
+    tersoff_sorted_ctas<T, Rec, BT, PCA, NT>(blockIdx.x, gridDim.x, s, tb, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tab,
+                                             types, list, count, Q, MASK, pe, f, virial, status);
+}
+
+// One element, rows of any length (config 5), ONE launch: the first `tail_ctas` CTAs run the loop code on the
+// bin of atoms with more than MR in-range neighbours (few atoms, but a tile of them is ~20 us of dependent
+// latency: they start first and overlap with everything else), the other CTAs run the register body on the
+// bin with at most MR, BT atoms each.  (Measured alternatives: the tail as a kernel of its own after the
+// register kernel costs its full latency, 25 us per step; on a second stream, the fork/join events cost more.)
+template <class T, class Rec, int MR, int BT, int PCA, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
+k_tersoff_hot(int64_t n, int tail_ctas, const double* __restrict__ x, const double* __restrict__ y,
+              const double* __restrict__ z, double Lx, double Ly, double Lz,
+              const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+              const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, 1> tab,
+              const int32_t* __restrict__ lists, const int32_t* __restrict__ counts,
+              const double* __restrict__ gtab, Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+              double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
+              int* __restrict__ status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
+    const fm::Tab tb = fm::stage_tables(s.tab, gtab);
+    __syncthreads();
+    if ((int)blockIdx.x < tail_ctas)
+        tersoff_sorted_ctas<T, Rec, BT, PCA, 1>(blockIdx.x, tail_ctas, s, tb, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tab,
+                                                nullptr, lists + 2 * n, counts + 2, Q, MASK, pe, f, virial, status);
+    else
+        tersoff_binned_cta<T, Rec, MR, BT>((int64_t)blockIdx.x - tail_ctas, n, x, y, z, Lx, Ly, Lz, NL, REV, lists,
+                                           counts, p, tb, Q, MASK, pe, f, virial);
 }
 
 template <class T>
@@ -643,18 +714,39 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
     TersoffTab<T, NT> tab;
     ps::RangeTab<T> rt;
     make_tab<T, NT>(mp, &tab, &rt);
-    nl->launches[MD_KIND_PAIR] += 1;
+    // One element: atoms with at most 4 in-range neighbours (bin 0: four in five of a hot crystal) go to the
+    // register kernel, the others (bin 2) to the loop kernel.  Several elements: the loop kernel takes all.
+    ps::Bins bins;
+    bins.b0 = 4; bins.b1 = 4;
+    bins.list = NT == 1 ? nl->bin_list : nullptr;
+    bins.count = nl->bin_count;
+    if (NT == 1) MD_CUDA_TRY(cudaMemsetAsync(nl->bin_count, 0, 4 * sizeof(int32_t), s));
+    nl->launches[MD_KIND_PAIR] += NT == 1 ? 2 : 1;
     ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2],
-                                                                 nl->NN, nl->NL, rt, NT > 1 ? types : nullptr, nl->MASK);
+                                                                 nl->NN, nl->NL, rt, NT > 1 ? types : nullptr, nl->MASK, bins);
     nl->q_dense = 1;
     constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
+    const unsigned grid = (unsigned)((n + BT - 1) / BT);      // sized for "every atom in this bin"; surplus CTAs exit at once
     using Sm = TersoffSortSmem<T, BT, PCA>;
-    auto kern = k_tersoff_sorted<T, Rec, BT, PCA, 4, 168, NT>;
+    auto kern = k_tersoff_sorted<T, Rec, BT, PCA, NT>;
     const int rca = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
     if (rca != MD_OK) return rca;
-    kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
-        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types, gtab, (Rec*)nl->Q, nl->MASK,
-        pe, f, virial, nl->d_status);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if constexpr (NT == 1) {
+        const int tail = sms;                                // one loop-code CTA per SM for the tail bin
+        auto hot = k_tersoff_hot<T, Rec, 4, BT, PCA, 168>;
+        const int rch = md_allow_dynamic_smem((const void*)hot, (int)sizeof(Sm));
+        if (rch != MD_OK) return rch;
+        hot<<<grid + (unsigned)tail, BT, sizeof(Sm), s>>>(n, tail, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV,
+                                                        p, tab, nl->bin_list, nl->bin_count, gtab, (Rec*)nl->Q, nl->MASK,
+                                                        pe, f, virial, nl->d_status);
+    } else {
+        kern<<<std::min<unsigned>(grid, 3u * (unsigned)sms), BT, sizeof(Sm), s>>>(
+            n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types, nullptr, nullptr, gtab,
+            (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status);
+    }
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
 }
