@@ -320,6 +320,7 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
         if (nl->n != n) return MD_ERR_NO_LIST;
         const bool last = step == first_step + nsteps - 1;
         vv.mode = last ? 1 : 2;
+        vv.pdl_pair = step % rebuild_every != 0;             // the list is the one the kernel before already used
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  last ? pe : nullptr, f, nullptr, nullptr, &vv, s)) != MD_OK) return rc;
     }

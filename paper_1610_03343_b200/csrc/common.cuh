@@ -95,7 +95,32 @@ struct VVFuse {
     int mode;
     double hk, dt;
     double *x, *y, *z, *vx, *vy, *vz;
+    int pdl_pair;   // 1: the kernel launched just before this step's pair phase was this loop's own k_gather_vv /
+                    // k_kick_drift and the list has not changed since (md_launch_pdl below)
 };
+
+// Programmatic dependent launch (sm_90+; md_nve_run only).  A kernel launched with `pdl` may start while the
+// kernel before it on the stream is draining its last CTAs: everything it does before md_grid_wait() overlaps
+// with that tail (and with the launch latency), so it may only READ there what the kernel before it does not
+// write.  md_grid_wait() returns when that kernel has completed and its writes are visible;
+// md_grid_release() lets the NEXT kernel on the stream be scheduled once every CTA of this one has called it.
+// Every kernel calls release only AFTER its own wait, so "the kernel before has completed" is transitive: when a
+// dependent starts, every earlier kernel of the stream is complete.  Launched without the attribute both calls
+// are no-ops.
+__device__ __forceinline__ void md_grid_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void md_grid_release() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+inline cudaError_t md_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                 bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
 
 // RAII scope: counts `nk` kernel launches of `kind` and, if profiling is on, brackets them with events.
 struct ProfScope {

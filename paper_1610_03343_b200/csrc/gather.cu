@@ -70,17 +70,22 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
 // k_kick_drift (integrate.cu), so the trajectory is bit-identical to the unfused composition.
 template <class T, class Rec, int MODE>
 __global__ void __launch_bounds__(256)
-k_gather_vv(int64_t n, const Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK, int dense,
-            double* __restrict__ f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
-            double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
+k_gather_vv(int64_t n, const Rec* Q, const unsigned long long* MASK, int dense,   // Q, MASK, f: no __restrict__/.nc --
+            double* f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,   // the pair kernel
+            double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,           // before wrote them
             double hk, double dt, double Lx, double Ly, double Lz) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    unsigned long long mask = MASK[i];
-    const double ox = f[i], oy = f[n + i], oz = f[2 * n + i];           // own halves sum_j P_ij
+    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = i0 < n ? i0 : n - 1;
+    // launched as a programmatic dependent of the pair kernel (common.cuh, md_launch_pdl): the velocity and
+    // position of the atom, which the pair kernel does not write, are requested while that kernel drains
     double ux = vx[i], uy = vy[i], uz = vz[i];
     double px = 0, py = 0, pz = 0;
     if (MODE == 2) { px = x[i]; py = y[i]; pz = z[i]; }
+    md_grid_wait();
+    md_grid_release();
+    if (i0 >= n) return;
+    unsigned long long mask = MASK[i];
+    const double ox = f[i], oy = f[n + i], oz = f[2 * n + i];           // own halves sum_j P_ij
     T Fx = T(0), Fy = T(0), Fz = T(0);
     if (dense) {                                             // popc(mask) consecutive slots
         const int cnt = __popcll(mask);
@@ -121,8 +126,9 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
 #define MD_GATHER_VV(TT, RR, MODE)                                                                        \
-    k_gather_vv<TT, RR, MODE><<<gb, 256, 0, s>>>(n, (const RR*)nl->Q, nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z,   \
-                                                 vv->vx, vv->vy, vv->vz, vv->hk, vv->dt, box[0], box[1], box[2])
+    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, true, n, (const RR*)nl->Q,            \
+                              nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z, vv->vx, vv->vy, vv->vz, vv->hk, vv->dt,    \
+                              box[0], box[1], box[2]))
         if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }
         else { if (vv->mode == 2) MD_GATHER_VV(double, PairRec64, 2); else MD_GATHER_VV(double, PairRec64, 1); }
 #undef MD_GATHER_VV

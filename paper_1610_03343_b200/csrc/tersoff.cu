@@ -323,8 +323,8 @@ tersoff_reg_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], un
 // Thread-per-atom kernel for crystal rows (at most MR listed entries): slot m is list position m.
 template <class T, class Rec, int MR, int BT, int MAXREG>
 __global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
-k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y,
-               const double* __restrict__ z, double Lx, double Ly, double Lz,
+k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__: see below
+               double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
@@ -346,6 +346,11 @@ k_tersoff_atom(int64_t n, int K, const double* __restrict__ x, const double* __r
         rv[m] = (int)REV[(int64_t)mk * n + i];
     }
     const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    // Inside md_nve_run this kernel is launched as a programmatic dependent of the fused gather kernel that
+    // wrote x, y, z (common.cuh, md_launch_pdl): the list loads above overlap with that kernel's tail; the
+    // coordinates are read only from here on, through plain (coherent, non-.nc) loads.
+    md_grid_wait();
+    md_grid_release();
     const double xi = x[i], yi = y[i], zi = z[i];
     double dx[MR], dy[MR], dz[MR];
 #pragma unroll
@@ -754,15 +759,15 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
 template <class T, class Rec>
 int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
            const double box[3], const md_tersoff_params* hp, double* pe, double* f, double* virial,
-           cudaStream_t s) {
+           bool pdl, cudaStream_t s) {
     const TersoffDev<T> p = make_dev<T>(hp);
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
 #define MD_TERSOFF_LAUNCH(MRV, BT, MAXREG)                                                                 \
-    k_tersoff_atom<T, Rec, MRV, BT, MAXREG><<<(unsigned)((n + BT - 1) / BT), BT, 0, s>>>(n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN,    \
-                                                         nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,          \
-                                                         nl->MASK, pe, f, virial, nl->d_status)
+    MD_CUDA_TRY(md_launch_pdl(k_tersoff_atom<T, Rec, MRV, BT, MAXREG>, dim3((unsigned)((n + BT - 1) / BT)), dim3(BT), 0, s, pdl, \
+                              n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab,   \
+                              (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status))
     // Kernel selection by the row lengths of the list (known on the host once per build): the register
     // kernel handles rows of up to 4 entries (the crystal) in its fast path and longer ones through a slow
     // per-thread fallback, so it is used while fewer than 1 row in 256 is longer; otherwise the
@@ -816,8 +821,9 @@ int md_launch_tersoff(md_neighbors* nl, int64_t n, const double* x, const double
                       const md_tersoff_params* p, int precision, double* pe, double* f, double* virial,
                       double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0) return MD_OK;
-    int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, s)
-                                  : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, s);
+    const bool pdl = vv && vv->pdl_pair;
+    int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, pdl, s)
+                                  : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, pdl, s);
     if (rc != MD_OK) return rc;
     return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, vv, s);
 }
