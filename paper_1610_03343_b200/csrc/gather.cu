@@ -69,8 +69,8 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
 // anything is stored.  The arithmetic is operation for operation that of k_gather followed by k_kick and
 // k_kick_drift (integrate.cu), so the trajectory is bit-identical to the unfused composition.
 template <class T, class Rec, int MODE>
-__global__ void __launch_bounds__(256)
-k_gather_vv(int64_t n, const Rec* Q, const unsigned long long* MASK, int dense,   // Q, MASK, f: no __restrict__/.nc --
+__global__ void __launch_bounds__(256, 4)
+k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int dense,   // Q, MASK, f: no __restrict__/.nc --
             double* f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,   // the pair kernel
             double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,           // before wrote them
             double hk, double dt, double Lx, double Ly, double Lz) {
@@ -84,17 +84,29 @@ k_gather_vv(int64_t n, const Rec* Q, const unsigned long long* MASK, int dense, 
     md_grid_wait();
     md_grid_release();
     if (i0 >= n) return;
+    // The first four record slots are requested before MASK has arrived (their addresses depend on i only): one
+    // dependent load level less.  A slot the mask does not select is loaded and dropped (it lies inside Q).
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+    T hx[4], hy[4], hz[4];
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl) rm::load_rec(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
     unsigned long long mask = MASK[i];
     const double ox = f[i], oy = f[n + i], oz = f[2 * n + i];           // own halves sum_j P_ij
-    T Fx = T(0), Fy = T(0), Fz = T(0);
     if (dense) {                                             // popc(mask) consecutive slots
         const int cnt = __popcll(mask);
-        for (int sl = 0; sl < cnt; ++sl) {
+#pragma unroll
+        for (int sl = 0; sl < 4; ++sl)
+            if (sl < cnt) { Fx += hx[sl]; Fy += hy[sl]; Fz += hz[sl]; }
+        for (int sl = 4; sl < cnt; ++sl) {
             T qx, qy, qz;
             rm::load_rec(&Q[(int64_t)sl * n + i], &qx, &qy, &qz);
             Fx += qx; Fy += qy; Fz += qz;
         }
-    } else {
+    } else {                                                 // slot = list position
+#pragma unroll
+        for (int sl = 0; sl < 4; ++sl)
+            if (mask >> sl & 1ull) { Fx += hx[sl]; Fy += hy[sl]; Fz += hz[sl]; }
+        mask &= ~15ull;
         while (mask) {
             const int m = __ffsll((long long)mask) - 1;
             mask &= mask - 1;
@@ -126,7 +138,7 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
 #define MD_GATHER_VV(TT, RR, MODE)                                                                        \
-    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, true, n, (const RR*)nl->Q,            \
+    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, true, n, nl->K, (const RR*)nl->Q,            \
                               nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z, vv->vx, vv->vy, vv->vz, vv->hk, vv->dt,    \
                               box[0], box[1], box[2]))
         if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }

@@ -194,27 +194,33 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
         if (ay < 0) { ay += g.nc[1]; ys += Lyf; } else if (ay >= g.nc[1]) { ay -= g.nc[1]; ys -= Lyf; }
         axs[o] = ax; xss[o] = xs; ays[o] = ay; yss[o] = ys;
     }
-    if (cz > 0 && cz < g.nc[2] - 1) {
-        // interior in z: the three z-neighbour cells of a column are contiguous in cell order, so the
-        // 27 cells are 9 ranges; all 18 bounds are fetched before the first scan
-        int beg[9], end[9];
+    // The z-neighbour cells of a column are contiguous in cell order, so the 27 cells are 9 ranges (the window
+    // cz-1..cz+1 clipped to the column) plus, for an atom in the first or last cell of its column, the 9 single
+    // cells on the far side of the periodic boundary.  All lanes walk the same loop structure: a lane without
+    // a wrapped part sees nine empty ranges there (a warp of 32 cell-ordered atoms spans ~15 of a column's cells,
+    // so every other warp holds such an atom; as a separate 27-range code path it cost those warps a second pass).
+    const int nz = g.nc[2];
+    const int zlo = cz > 0 ? cz - 1 : 0, zhi = cz < nz - 1 ? cz + 1 : nz - 1;
+    int beg[9], end[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) {                            // all 18 bounds are fetched before the first scan
+        const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * nz;
+        beg[c] = cell_start[base + zlo];
+        end[c] = cell_start[base + zhi + 1];
+    }
+#pragma unroll
+    for (int c = 0; c < 9; ++c) scan(beg[c], end[c], xss[c / 3], yss[c % 3], zf);
+    if (cz == 0 || cz == nz - 1) {
+        const int wz = cz == 0 ? nz - 1 : 0;
+        const float zs = cz == 0 ? zf + Lzf : zf - Lzf;
 #pragma unroll
         for (int c = 0; c < 9; ++c) {
-            const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * g.nc[2] + cz;
-            beg[c] = cell_start[base - 1];
-            end[c] = cell_start[base + 2];
+            const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * nz + wz;
+            beg[c] = cell_start[base];
+            end[c] = cell_start[base + 1];
         }
 #pragma unroll
-        for (int c = 0; c < 9; ++c) scan(beg[c], end[c], xss[c / 3], yss[c % 3], zf);
-    } else {
-        for (int c = 0; c < 9; ++c) {
-            const int base = (axs[c / 3] * g.nc[1] + ays[c % 3]) * g.nc[2];
-            for (int oz = -1; oz <= 1; ++oz) {
-                int az = cz + oz; float zs = zf;
-                if (az < 0) { az += g.nc[2]; zs += Lzf; } else if (az >= g.nc[2]) { az -= g.nc[2]; zs -= Lzf; }
-                scan(cell_start[base + az], cell_start[base + az + 1], xss[c / 3], yss[c % 3], zs);
-            }
-        }
+        for (int c = 0; c < 9; ++c) scan(beg[c], end[c], xss[c / 3], yss[c % 3], zs);
     }
     {   // longest row: one atomic per warp
         const unsigned act = __activemask();
