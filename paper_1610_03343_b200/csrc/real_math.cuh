@@ -22,6 +22,17 @@ __device__ __forceinline__ void sincos(float a, float* s, float* c) { ::sincosf(
 __device__ __forceinline__ void store_rec(PairRec64* q, double px, double py, double pz) {
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(q), "d"(px), "d"(py), "d"(pz), "d"(0.0) : "memory");
 }
+// The same record as two 128-bit stores, for code inside a non-inlined device function: ptxas 12.9 turned the
+// 256-bit store above into a single 64-bit one (only Px reached memory) when tersoff_pair_generic was compiled
+// as a callee of the 128-register kernel k_tersoff_lean (seen in the SASS and as stale records on the GPU).
+__device__ __forceinline__ void store_rec_2x128(PairRec64* q, double px, double py, double pz) {
+    double2* d = reinterpret_cast<double2*>(q);
+    d[0] = make_double2(px, py);
+    d[1] = make_double2(pz, 0.0);
+}
+__device__ __forceinline__ void store_rec_2x128(float4* q, float px, float py, float pz) {
+    *q = make_float4(px, py, pz, 0.f);
+}
 __device__ __forceinline__ void store_rec(float4* q, float px, float py, float pz) {
     *q = make_float4(px, py, pz, 0.f);
 }

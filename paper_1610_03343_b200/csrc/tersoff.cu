@@ -31,6 +31,12 @@ template <class T> struct TsPair { T A, B, lambda, mu, R, w, chi; };     // w = 
 template <class T> struct TsCenter { T beta, n, h, c2, d2, c2_over_d2, minus_half_over_n; };
 template <class T, int NT> struct TersoffTab { TsCenter<T> c[NT]; TsPair<T> p[NT * NT]; };
 
+#ifndef LEAN_DEBUG_SLOW
+#define LEAN_DEBUG_SLOW false
+#endif
+#ifndef MD_TERSOFF_LEAN_MAXREG
+#define MD_TERSOFF_LEAN_MAXREG 128   // 4 CTAs of 128 threads per SM
+#endif
 constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom (generic path)
 
 // Generic path: any number of in-range neighbours up to TERSOFF_KC, per-thread arrays in local memory.
@@ -139,7 +145,7 @@ tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const d
     for (int a = 0; a < M; ++a) {
         const int m = slot[a];
         const int mm = REV[(int64_t)m * n + i];
-        rm::store_rec(&Q[(int64_t)mm * n + jdx[a]], Px[a], Py[a], Pz[a]);
+        rm::store_rec_2x128(&Q[(int64_t)mm * n + jdx[a]], Px[a], Py[a], Pz[a]);   // see real_math.cuh
         Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
         if (virial) {
             const T rx = ex[a] * r[a], ry = ey[a] * r[a], rz = ez[a] * r[a];
@@ -389,6 +395,197 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
     }
     MASK[i] = (unsigned long long)mask;
     tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Lean register body: the crystal case of the NVE loop and of force-only calls (no virial asked for, no pair
+// inside the cut-off window R < r < S).  Then f_C is 1 or 0 and f_C' = 0 for every slot, so f_C, f_C', r and
+// every term that carries f_C' drop out (in the force pass g itself is no longer needed, only g'), the partner
+// index and reverse slot fold into ONE 32-bit record index per slot, and the body fits 128 registers: 4 CTAs
+// of 128 threads per SM instead of 3 (the kernel is bound by latency, not by the FP64 pipe: ncu r02a).  An
+// atom with a pair inside the window is handed to the general per-thread path before any arithmetic.
+template <class T, class Rec, int MR>
+__device__ __forceinline__ void
+tersoff_lean_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], const T (&d2in)[MR], unsigned mask,
+                  const unsigned (&qi)[MR], const TersoffDev<T>& p, const fm::Tab& tb,
+                  Rec* __restrict__ Q, double* __restrict__ pe, double* __restrict__ f) {
+    constexpr int NP = MR * (MR - 1) / 2;
+    T rinv[MR], fR[MR], fA[MR], zeta[MR];
+    {
+        T d2s[MR], rr[MR], aR[MR], aA[MR];
+#pragma unroll
+        for (int m = 0; m < MR; ++m) d2s[m] = (mask >> m & 1u) ? d2in[m] : T(1);   // keeps an empty slot finite
+        fm::rsqrt_v<MR>(d2s, rinv);
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            rr[m] = d2s[m] * rinv[m];
+            ex[m] *= rinv[m]; ey[m] *= rinv[m]; ez[m] *= rinv[m];
+            aR[m] = -p.lambda * rr[m]; aA[m] = -p.mu * rr[m];
+        }
+        fm::exp_v<MR>(aR, fR, tb);
+        fm::exp_v<MR>(aA, fA, tb);
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            const bool in = mask >> m & 1u;
+            fR[m] = in ? p.A * fR[m] : T(0);
+            fA[m] = in ? p.B * fA[m] : T(0);
+            zeta[m] = T(0);
+        }
+    }
+    // zeta (Eq. 4) with f_C = 1 inside the range: unordered slot pairs once (g_ijk = g_ikj for one element)
+    {
+        T x2[NP], den[NP], q[NP];
+        int c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T xx = p.h - (ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b]);
+                x2[c] = xx * xx;
+                den[c] = p.d2 + x2[c];
+            }
+        fm::rcp_v<NP>(den, q);
+        c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T g = T(1) + p.c2_over_d2 * x2[c] * q[c];
+                zeta[a] += (mask >> b & 1u) ? g : T(0);
+                zeta[b] += (mask >> a & 1u) ? g : T(0);
+            }
+    }
+    // b, b' (Eq. 3); U_i; D_a = (mu b f_A - lambda f_R)/2; h_a = -f_A b'/2  (all zero for a slot out of range)
+    T U = T(0);
+    T Px[MR], Py[MR], Pz[MR], hh[MR];
+    {
+        T zt[MR], w1[MR], w2[MR], t[MR], u[MR], bb[MR], rc[MR];
+#pragma unroll
+        for (int a = 0; a < MR; ++a) { zt[a] = zeta[a] > T(0) ? zeta[a] : T(1); w1[a] = p.beta * zt[a]; }
+        fm::log_v<MR>(w1, w2, tb);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) w2[a] *= p.n;
+        fm::exp_v<MR>(w2, t, tb);                                        // (beta zeta)^n
+#pragma unroll
+        for (int a = 0; a < MR; ++a) { u[a] = T(1) + t[a]; w1[a] = zt[a] * u[a]; }
+        fm::log_v<MR>(u, w2, tb);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) w2[a] *= p.minus_half_over_n;
+        fm::exp_v<MR>(w2, bb, tb);                                       // (1 + t)^(-1/2n)
+        fm::rcp_v<MR>(w1, rc);
+#pragma unroll
+        for (int a = 0; a < MR; ++a) {
+            const bool pos = zeta[a] > T(0);                             // zeta = 0: b = 1, b' = 0 (reading A8)
+            const T b = pos ? bb[a] : T(1);
+            const T bp = pos ? T(-0.5) * bb[a] * t[a] * rc[a] : T(0);
+            const T bfA = b * fA[a];
+            U += T(0.5) * (fR[a] - bfA);
+            const T D = T(0.5) * (p.mu * bfA - p.lambda * fR[a]);
+            hh[a] = T(-0.5) * fA[a] * bp;
+            Px[a] = D * ex[a]; Py[a] = D * ey[a]; Pz[a] = D * ez[a];
+        }
+    }
+    // P_a = D_a e_a + sum_{b != a} (h_a [b in range] + h_b [a in range]) g'_ab (e_b - cos e_a)/r_a
+    {
+        T cs[NP], xx[NP], den[NP], q[NP];
+        int c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                cs[c] = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
+                xx[c] = p.h - cs[c];
+                den[c] = p.d2 + xx[c] * xx[c];
+            }
+        fm::rcp_v<NP>(den, q);
+        c = 0;
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+#pragma unroll
+            for (int b = a + 1; b < MR; ++b, ++c) {
+                const T gp = T(-2) * p.c2 * xx[c] * q[c] * q[c];         // dg/dcos
+                const T tab = (((mask >> b & 1u) ? hh[a] : T(0)) + ((mask >> a & 1u) ? hh[b] : T(0))) * gp;
+                const T ta = tab * rinv[a], tb2 = tab * rinv[b];
+                const T ua = -ta * cs[c], ub = -tb2 * cs[c];
+                Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
+                Px[b] += tb2 * ex[a] + ub * ex[b]; Py[b] += tb2 * ey[a] + ub * ey[b]; Pz[b] += tb2 * ez[a] + ub * ez[b];
+            }
+    }
+    T Fx = T(0), Fy = T(0), Fz = T(0);
+#pragma unroll
+    for (int a = 0; a < MR; ++a)
+        if (mask >> a & 1u) {
+            rm::store_rec(&Q[qi[a]], Px[a], Py[a], Pz[a]);
+            Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
+        }
+    if (pe) pe[i] = (double)U;
+    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+}
+
+template <class T, class Rec, int MR, int BT, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
+k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__: as k_tersoff_atom
+               double Lx, double Ly, double Lz,
+               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
+               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+               double* __restrict__ pe, double* __restrict__ f, int* __restrict__ status) {
+    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = i0 < n ? i0 : n - 1;
+    const int nn = NN[i];
+    int jd[MR];
+    unsigned qi[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) {
+        const int mk = m < K ? m : 0;
+        const int jr = NL[(int64_t)mk * n + i];
+        jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
+        qi[m] = (unsigned)REV[(int64_t)mk * n + i] * (unsigned)n + (unsigned)jd[m];   // n * K <= 2e9 (md_neighbors_create)
+    }
+    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    md_grid_wait();                                          // programmatic dependent of the fused gather (see k_tersoff_atom)
+    md_grid_release();
+    const double xi = x[i], yi = y[i], zi = z[i];
+    double dx[MR], dy[MR], dz[MR];
+#pragma unroll
+    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }
+    __syncthreads();
+    if (i0 >= n) return;
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
+    T ex[MR], ey[MR], ez[MR], d2[MR];
+    unsigned mask = 0u;
+    bool slow = nn > MR || LEAN_DEBUG_SLOW;
+    {
+        bool far = false;
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            dx[m] -= xi; dy[m] -= yi; dz[m] -= zi;
+            d2[m] = ps::in_range_d2((T)dx[m], (T)dy[m], (T)dz[m]);       // the one in-range decision (pair_sort.cuh)
+            far = far || mi.far(d2[m]);
+        }
+        if (__any_sync(__activemask(), far)) {               // warp-uniform: interior warps never shift
+#pragma unroll
+            for (int m = 0; m < MR; ++m) {
+                mi.wrap(dx[m], dy[m], dz[m]);
+                d2[m] = ps::in_range_d2((T)dx[m], (T)dy[m], (T)dz[m]);
+            }
+        }
+        const T R2 = p.R * p.R;
+#pragma unroll
+        for (int m = 0; m < MR; ++m) {
+            ex[m] = (T)dx[m]; ey[m] = (T)dy[m]; ez[m] = (T)dz[m];
+            const bool in = m < nn && d2[m] < p.S2;
+            mask |= in ? 1u << m : 0u;
+            slow = slow || (in && d2[m] > R2);               // a pair inside the cut-off window
+        }
+    }
+    if (slow) {                                              // rows longer than MR, or f_C not 0/1: the general path
+        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, nullptr, status);
+        return;
+    }
+    MASK[i] = (unsigned long long)mask;
+    tersoff_lean_body<T, Rec, MR>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f);
 }
 
 // Register path for a bin of atoms with at most MR in-range neighbours (pair_sort.cuh, Bins): thread t of CTA
@@ -781,6 +978,12 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, &one, nullptr, gtab, pe, f, virial, s);
     }
     nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
+    if (!virial) {                                           // NVE loop and force-only calls: the lean body
+        MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, 128, MD_TERSOFF_LEAN_MAXREG>, dim3((unsigned)((n + 127) / 128)),
+                                  dim3(128), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
+                                  nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, nl->d_status));
+        return MD_OK;
+    }
     MD_TERSOFF_LAUNCH(4, 128, 168);
 #undef MD_TERSOFF_LAUNCH
     MD_CUDA_TRY(cudaGetLastError());

@@ -78,6 +78,37 @@ def test_force_with_imported_oracle_list_and_optional_outputs():
     assert (only_pe["pe"] == full["pe"]).all()
 
 
+def test_lean_register_kernel_next_to_general_path_atoms():
+    """Force-only calls on a crystal use the 128-register lean kernel (no f_C terms); atoms with a list row longer
+    than 4 or with a pair inside the cut-off window R < r < S take the general per-thread path inside the same
+    launch, and their partners gather the records it pushes.  One atom is displaced so that both cases occur."""
+    s = mi.silicon_crystal(8, 0.05, 300.0, 21)
+    p = mi.TERSOFF_SI_C
+    i = 1234
+    NN0, NL0 = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list("tersoff"), 16)
+    j = NL0[i][0]
+    d = np.array([s[k][j] - s[k][i] for k in "xyz"])
+    d -= s["box"] * np.round(d / s["box"])
+    shift = -(0.5 / np.linalg.norm(d)) * d                    # stretch the bond i-j from ~2.35 A to ~2.85 A
+    for a, k in enumerate("xyz"):
+        s[k][i] = (s[k][i] + shift[a]) % s["box"][a]
+    g = GpuSystem(s, 16)
+    g.build(mi.r_list("tersoff"))
+    max_row, long_rows = md.md_neighbors_row_stats(g.nl)
+    NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list("tersoff"), 16)
+    ref = oracle.evaluate("tersoff", p, s["x"], s["y"], s["z"], s["box"], NN, NL, precision="f80", want=("pe", "f"))
+    dij = np.array([s[k][j] - s[k][i] for k in "xyz"])
+    dij -= s["box"] * np.round(dij / s["box"])
+    assert p["R"] < np.linalg.norm(dij) < p["S"]             # a window pair exists
+    assert max_row > 4 and 0 < long_rows and long_rows * 256 <= g.n   # long rows exist, register kernel still chosen
+    for _ in range(2):                                        # twice: a stale record of the first call must not help
+        out = g.force("tersoff", p, want=("pe", "f"))
+        assert_close_fp64("f", out["f"], ref["f"])
+        assert_close_energy(out["pe"], ref["pe"])
+    full = g.force("tersoff", p)                              # the 168-register kernel (virial asked for)
+    assert_close_fp64("f", full["f"], ref["f"])
+
+
 def test_run_to_run_bitwise_reproducible():
     s = mi.silicon_crystal(6, 0.15, 1500.0, 77)
     a = GpuSystem(s, 16); a.build(3.5); oa = a.force("tersoff", mi.TERSOFF_SI_C)
