@@ -37,130 +37,161 @@ template <class T, int NT> struct TersoffTab { TsCenter<T> c[NT]; TsPair<T> p[NT
 #ifndef MD_TERSOFF_LEAN_MAXREG
 #define MD_TERSOFF_LEAN_MAXREG 128   // 4 CTAs of 128 threads per SM
 #endif
-constexpr int TERSOFF_KC = 16;   // cap on in-range neighbours per atom (generic path)
 
-// Generic path: any number of in-range neighbours up to TERSOFF_KC, per-thread arrays in local memory.
-// Used by threads whose list row is longer than the register path's MR slots.
+// General path, one WARP per atom: list rows of any length (up to 64 listed, 32 in range) and pairs inside the
+// cut-off window.  The register kernels hand it the few atoms their straight-line bodies do not cover.  Such an
+// atom used to be finished by its own thread alone (per-thread arrays in local memory, ~2500 dependent
+// instructions: one 8 us straggler held an SM long after the other 147 had finished a 35 us kernel -- ncu
+// l1tex__cycles_active min/avg/max, profiles/r02b).  Here the lanes of a warp are the atom's in-range slots:
+//   screen   lane l tests list entries l and l + 32; the in-range ones are compacted to lanes 0..M-1 through a
+//            per-warp shared-memory scratch (ballot + popc ranks);
+//   pass 1   lane a: e_a, 1/r_a, f_C, f_C', f_R, f_A of its slot;
+//   pass 2   lane a: zeta_a = sum_{b != a} f_C(r_b) g_ab with slot b's data fetched by shuffles; b, b', D_a, h_a;
+//   pass 3   lane a: P_a (T5) likewise, stored to Q[rev(i,a) * n + j_a]; U_i and the own halves by a shuffle tree.
+// Called by all 32 lanes of a warp (converged).  Records are stored as 2 x 128 bit (real_math.cuh).
+struct WarpSlots { double dx[32], dy[32], dz[32]; int j[32], m[32]; };
+
+template <class T>
+__device__ __forceinline__ T warp_sum(T v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
 template <class T, class Rec>
 __device__ __noinline__ void
-tersoff_pair_generic(int64_t i, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
-               const double* __restrict__ z, double Lx, double Ly, double Lz,
-               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, TersoffDev<T> p,
-               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-               int* __restrict__ status) {
+tersoff_warp_atom(int64_t i, int64_t n, const double* x, const double* y, const double* z, double Lx, double Ly,
+                  double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                  const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const fm::Tab& tb, Rec* __restrict__ Q,
+                  unsigned long long* __restrict__ MASK, double* __restrict__ pe, double* __restrict__ f,
+                  double* __restrict__ virial, int* __restrict__ status, WarpSlots& ws) {
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
+    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
+    const int nn = min(NN[i], 64);
     const double xi = x[i], yi = y[i], zi = z[i];
-    const double hx = 0.5 * Lx, hy = 0.5 * Ly, hz = 0.5 * Lz;
-    const int nn = NN[i];
-
-    T ex[TERSOFF_KC], ey[TERSOFF_KC], ez[TERSOFF_KC], r[TERSOFF_KC];
-    T fc[TERSOFF_KC], fcp[TERSOFF_KC], fR[TERSOFF_KC], fA[TERSOFF_KC];
-    T zeta[TERSOFF_KC];
-    int jdx[TERSOFF_KC];
-    unsigned char slot[TERSOFF_KC];
-    int M = 0;
-    unsigned long long mask = 0ull;
-
-    for (int m = 0; m < nn; ++m) {
-        const int j = NL[(int64_t)m * n + i];
-        const double dx = md_min_image(x[j] - xi, Lx, hx);
-        const double dy = md_min_image(y[j] - yi, Ly, hy);
-        const double dz = md_min_image(z[j] - zi, Lz, hz);
-        const T tx = (T)dx, ty = (T)dy, tz = (T)dz;
-        const T d2 = ps::in_range_d2(tx, ty, tz);
-        if (d2 < p.S2) {
-            if (M >= TERSOFF_KC) { atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); continue; }
-            const T rinv = rm::rsqrt(d2);
-            const T rr = d2 * rinv;
-            ex[M] = tx * rinv; ey[M] = ty * rinv; ez[M] = tz * rinv; r[M] = rr;
-            T c = T(1), cp = T(0);
-            if (rr > p.R) {                                  // f_C window R < r < S (reading A1)
-                T sn, cs;
-                rm::sincos((rr - p.R) * p.w, &sn, &cs);
-                c = T(0.5) + T(0.5) * cs;
-                cp = T(-0.5) * p.w * sn;
-            }
-            fc[M] = c; fcp[M] = cp;
-            fR[M] = p.A * rm::exp(-p.lambda * rr);
-            fA[M] = p.B * rm::exp(-p.mu * rr);
-            zeta[M] = T(0);
-            jdx[M] = j; slot[M] = (unsigned char)m;
-            mask |= 1ull << m;
-            ++M;
-        }
-    }
-
-    // zeta_ij = sum_{k != j} f_C(r_ik) g_ijk (Eq. 4); single element: g_ijk = g_ikj, visit a < b once.
-    // g = 1 + (c/d)^2 x^2/(d^2 + x^2), x = h - cos (algebraically Eq. 5, without its cancellation)
-    for (int a = 0; a < M; ++a)
-        for (int b = a + 1; b < M; ++b) {
-            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-            const T xx = p.h - cs;
-            const T x2 = xx * xx;
-            const T g = T(1) + p.c2_over_d2 * x2 / (p.d2 + x2);
-            zeta[a] += fc[b] * g;
-            zeta[b] += fc[a] * g;
-        }
-
-    // b_ij, b'_ij (Eq. 3) and the two-body coefficients
-    T U = T(0);
-    T D[TERSOFF_KC], hh[TERSOFF_KC];
-    for (int a = 0; a < M; ++a) {
-        T b = T(1), bp = T(0);
-        const T zt = zeta[a];
-        if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
-            const T t = rm::exp(p.n * rm::log(p.beta * zt)); // (beta zeta)^n
-            b = rm::exp(p.minus_half_over_n * rm::log1p(t));
-            bp = -b * t / (T(2) * zt * (T(1) + t));
-        }
-        const T bfA = b * fA[a];
-        U += T(0.5) * fc[a] * (fR[a] - bfA);
-        D[a] = T(0.5) * (fcp[a] * (fR[a] - bfA) + fc[a] * (p.mu * bfA - p.lambda * fR[a]));
-        hh[a] = T(-0.5) * fc[a] * fA[a] * bp;
-    }
-
-    // P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g'_ab (e_b - cos e_a)/r_a + h_b fc'_a g_ab e_a ]
-    T Px[TERSOFF_KC], Py[TERSOFF_KC], Pz[TERSOFF_KC];
-    for (int a = 0; a < M; ++a) { Px[a] = D[a] * ex[a]; Py[a] = D[a] * ey[a]; Pz[a] = D[a] * ez[a]; }
-    for (int a = 0; a < M; ++a)
-        for (int b = a + 1; b < M; ++b) {
-            const T cs = ex[a] * ex[b] + ey[a] * ey[b] + ez[a] * ez[b];
-            const T xx = p.h - cs;
-            const T x2 = xx * xx;
-            const T q = T(1) / (p.d2 + x2);
-            const T g = T(1) + p.c2_over_d2 * x2 * q;
-            const T gp = T(-2) * p.c2 * xx * q * q;          // dg/dcos
-            const T tab = (hh[a] * fc[b] + hh[b] * fc[a]) * gp;
-            const T ta = tab / r[a], tb = tab / r[b];
-            const T ua = hh[b] * fcp[a] * g - ta * cs;       // coefficient of e_a in P_a
-            const T ub = hh[a] * fcp[b] * g - tb * cs;       // coefficient of e_b in P_b
-            Px[a] += ta * ex[b] + ua * ex[a]; Py[a] += ta * ey[b] + ua * ey[a]; Pz[a] += ta * ez[b] + ua * ez[a];
-            Px[b] += tb * ex[a] + ub * ex[b]; Py[b] += tb * ey[a] + ub * ey[b]; Pz[b] += tb * ez[a] + ub * ez[b];
-        }
-
-    // push P_ij to atom j's slot, accumulate the own halves
-    T Fx = T(0), Fy = T(0), Fz = T(0);
-    T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
-    for (int a = 0; a < M; ++a) {
-        const int m = slot[a];
-        const int mm = REV[(int64_t)m * n + i];
-        rm::store_rec_2x128(&Q[(int64_t)mm * n + jdx[a]], Px[a], Py[a], Pz[a]);   // see real_math.cuh
-        Fx += Px[a]; Fy += Py[a]; Fz += Pz[a];
-        if (virial) {
-            const T rx = ex[a] * r[a], ry = ey[a] * r[a], rz = ez[a] * r[a];
-            W[0] += rx * Px[a]; W[1] += rx * Py[a]; W[2] += rx * Pz[a];
-            W[3] += ry * Px[a]; W[4] += ry * Py[a]; W[5] += ry * Pz[a];
-            W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
-        }
-    }
-    MASK[i] = mask;
-    if (pe) pe[i] = (double)U;
-    if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
-    if (virial) {
+    // screen and compaction
+    bool in[2];
+    double qx[2], qy[2], qz[2];
+    int jj[2];
 #pragma unroll
-        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+    for (int h = 0; h < 2; ++h) {
+        const int m = lane + 32 * h;
+        const bool valid = m < nn;
+        jj[h] = valid ? NL[(int64_t)m * n + i] : (int)i;
+        qx[h] = x[jj[h]] - xi; qy[h] = y[jj[h]] - yi; qz[h] = z[jj[h]] - zi;
+        mi.wrap(qx[h], qy[h], qz[h]);
+        in[h] = valid && ps::in_range_d2((T)qx[h], (T)qy[h], (T)qz[h]) < p.S2;
     }
+    const unsigned lo = __ballot_sync(0xffffffffu, in[0]), hi = __ballot_sync(0xffffffffu, in[1]);
+    int M = __popc(lo) + __popc(hi);
+    if (M > 32) { if (lane == 0) atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); M = 32; }
+    __syncwarp();
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int rank = h == 0 ? __popc(lo & lt) : __popc(lo) + __popc(hi & lt);
+        if (in[h] && rank < 32) {
+            ws.dx[rank] = qx[h]; ws.dy[rank] = qy[h]; ws.dz[rank] = qz[h];
+            ws.j[rank] = jj[h]; ws.m[rank] = lane + 32 * h;
+        }
+    }
+    __syncwarp();
+    const bool act = lane < M;
+    // pass 1 (an idle lane computes on a unit vector and carries f_C = f_R = f_A = 0)
+    const T tx = act ? (T)ws.dx[lane] : T(1), ty = act ? (T)ws.dy[lane] : T(0), tz = act ? (T)ws.dz[lane] : T(0);
+    const int ja = act ? ws.j[lane] : 0, ma = act ? ws.m[lane] : 0;
+    const T d2 = ps::in_range_d2(tx, ty, tz);
+    const T rinv = fm::rsqrt(d2);
+    const T r = d2 * rinv;
+    const T ex = tx * rinv, ey = ty * rinv, ez = tz * rinv;
+    T fc = act ? T(1) : T(0), fcp = T(0);
+    if (act && r > p.R) {                                    // f_C window R < r < S (reading A1)
+        T sn, cs;
+        fm::sincos_0_pi((r - p.R) * p.w, &sn, &cs);
+        fc = T(0.5) + T(0.5) * cs;
+        fcp = T(-0.5) * p.w * sn;
+    }
+    const T fR = act ? p.A * fm::exp(-p.lambda * r, tb) : T(0);
+    const T fA = act ? p.B * fm::exp(-p.mu * r, tb) : T(0);
+    // pass 2: zeta (Eq. 4), g = 1 + (c/d)^2 x^2/(d^2 + x^2), x = h - cos (Eq. 5 without its cancellation)
+    T zt = T(0);
+    for (int b = 0; b < M; ++b) {
+        const T bx = __shfl_sync(0xffffffffu, ex, b), by = __shfl_sync(0xffffffffu, ey, b),
+                bz = __shfl_sync(0xffffffffu, ez, b), fcb = __shfl_sync(0xffffffffu, fc, b);
+        const T xx = p.h - (ex * bx + ey * by + ez * bz);
+        const T x2 = xx * xx;
+        const T g = T(1) + p.c2_over_d2 * x2 * fm::rcp(p.d2 + x2);
+        zt += b != lane ? fcb * g : T(0);
+    }
+    T bo = T(1), bp = T(0);
+    if (zt > T(0)) {                                         // zeta = 0: b = 1, b' = 0 (reading A8)
+        const T tt = fm::exp(p.n * fm::log(p.beta * zt, tb), tb);                 // (beta zeta)^n
+        bo = fm::exp(p.minus_half_over_n * fm::log(T(1) + tt, tb), tb);           // Eq. (3)
+        bp = T(-0.5) * bo * tt * fm::rcp(zt * (T(1) + tt));
+    }
+    const T bfA = bo * fA;
+    T U = T(0.5) * fc * (fR - bfA);                                               // U_ia / 2
+    const T D = T(0.5) * (fcp * (fR - bfA) + fc * (p.mu * bfA - p.lambda * fR));
+    const T hh = T(-0.5) * fc * fA * bp;
+    // pass 3: P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g' (e_b - cos e_a)/r_a + h_b fc'_a g e_a ]
+    T ce = D, sx = T(0), sy = T(0), sz = T(0);
+    for (int b = 0; b < M; ++b) {
+        const T bx = __shfl_sync(0xffffffffu, ex, b), by = __shfl_sync(0xffffffffu, ey, b),
+                bz = __shfl_sync(0xffffffffu, ez, b), fcb = __shfl_sync(0xffffffffu, fc, b),
+                hb = __shfl_sync(0xffffffffu, hh, b);
+        const T cs = ex * bx + ey * by + ez * bz;
+        const T xx = p.h - cs;
+        const T x2 = xx * xx;
+        const T q = fm::rcp(p.d2 + x2);
+        const T gp = T(-2) * p.c2 * xx * q * q;              // dg/dcos
+        const T ta = b != lane ? (hh * fcb + hb * fc) * gp * rinv : T(0);
+        ce += b != lane ? hb * fcp * (T(1) + p.c2_over_d2 * x2 * q) - ta * cs : T(0);
+        sx += ta * bx; sy += ta * by; sz += ta * bz;
+    }
+    T px = sx + ce * ex, py = sy + ce * ey, pz = sz + ce * ez;
+    if (act) {
+        const int rev = (int)REV[(int64_t)ma * n + i];
+        rm::store_rec_2x128(&Q[(int64_t)rev * n + ja], px, py, pz);
+    } else {
+        px = T(0); py = T(0); pz = T(0); U = T(0);
+    }
+    // U_i and the own halves: shuffle tree (fixed order)
+    const T Us = warp_sum(U), Fx = warp_sum(px), Fy = warp_sum(py), Fz = warp_sum(pz);
+    if (virial) {
+        const T rr = fm::rcp(rinv);
+        const T rx = ex * rr, ry = ey * rr, rz = ez * rr;
+        const T w[9] = {rx * px, rx * py, rx * pz, ry * px, ry * py, ry * pz, rz * px, rz * py, rz * pz};
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+            const T ws9 = warp_sum(w[k]);
+            if (lane == 0) virial[(int64_t)k * n + i] = (double)(T(-0.5) * ws9);
+        }
+    }
+    if (lane == 0) {
+        MASK[i] = (unsigned long long)lo | ((unsigned long long)hi << 32);
+        if (pe) pe[i] = (double)Us;
+        if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+    }
+    __syncwarp();                                            // the scratch may be reused by the caller's next atom
+}
+
+// The CTA's atoms that need the general path are queued (a shared-memory counter; the order in the queue does
+// not influence any result) and, after a barrier, taken one per warp.
+template <int BT>
+struct SlowQueue { WarpSlots ws[BT / 32]; int atom[BT]; int count; };
+
+template <class T, class Rec, int BT>
+__device__ __forceinline__ void
+tersoff_drain_queue(SlowQueue<BT>& sq, int64_t n, const double* x, const double* y, const double* z, double Lx,
+                    double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+                    const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const fm::Tab& tb, Rec* __restrict__ Q,
+                    unsigned long long* __restrict__ MASK, double* __restrict__ pe, double* __restrict__ f,
+                    double* __restrict__ virial, int* __restrict__ status) {
+    __syncthreads();
+    const int ns = sq.count, w = threadIdx.x >> 5;
+    for (int k = w; k < ns; k += BT / 32)
+        tersoff_warp_atom<T, Rec>(sq.atom[k], n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, virial, status,
+                                  sq.ws[w]);
 }
 
 // Register body: up to MR neighbour slots, every per-neighbour quantity in registers (all array indices are
@@ -340,6 +371,8 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
     // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
     // index and masked out below), and the table staging's barrier comes after the loads are in flight.
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    __shared__ SlowQueue<BT> s_slow;
+    if (threadIdx.x == 0) s_slow.count = 0;
     const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t i = i0 < n ? i0 : n - 1;
     const int nn = NN[i];
@@ -362,11 +395,8 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
 #pragma unroll
     for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
     __syncthreads();
-    if (i0 >= n) return;
-    if (nn > MR) {
-        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, virial, status);
-        return;
-    }
+    if (i0 < n && nn > MR) s_slow.atom[atomicAdd(&s_slow.count, 1)] = (int)i;   // rows longer than MR: the general path
+    if (i0 < n && nn <= MR) {
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
     T ex[MR], ey[MR], ez[MR];
     unsigned mask = 0u;
@@ -395,6 +425,8 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
     }
     MASK[i] = (unsigned long long)mask;
     tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
+    }
+    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, virial, status);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -531,6 +563,8 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, int* __restrict__ status) {
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    __shared__ SlowQueue<BT> s_slow;
+    if (threadIdx.x == 0) s_slow.count = 0;
     const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t i = i0 < n ? i0 : n - 1;
     const int nn = NN[i];
@@ -551,7 +585,7 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
 #pragma unroll
     for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }
     __syncthreads();
-    if (i0 >= n) return;
+    if (i0 < n) {
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
     T ex[MR], ey[MR], ez[MR], d2[MR];
     unsigned mask = 0u;
@@ -581,11 +615,13 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
         }
     }
     if (slow) {                                              // rows longer than MR, or f_C not 0/1: the general path
-        tersoff_pair_generic<T, Rec>(i, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, Q, MASK, pe, f, nullptr, status);
-        return;
+        s_slow.atom[atomicAdd(&s_slow.count, 1)] = (int)i;
+    } else {
+        MASK[i] = (unsigned long long)mask;
+        tersoff_lean_body<T, Rec, MR>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f);
     }
-    MASK[i] = (unsigned long long)mask;
-    tersoff_lean_body<T, Rec, MR>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f);
+    }
+    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, nullptr, status);
 }
 
 // Register path for a bin of atoms with at most MR in-range neighbours (pair_sort.cuh, Bins): thread t of CTA
