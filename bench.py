@@ -161,7 +161,8 @@ def main_reference(args):
 
 
 def traffic_from_profiles(kernel):
-    """dram bytes per launch of `kernel` from the committed ncu summary (data file, not code)."""
+    """dram bytes per launch of `kernel` from the committed ncu summary (data file, not code); measured at
+    512 000 atoms, so None for any other size."""
     try:
         t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
         return t.get(kernel)
@@ -221,7 +222,8 @@ def kernel_name(md, nl, pot, n):
     if pot == "sw":
         return "k_screen+k_sw_sorted"
     _, long_rows = md.md_neighbors_row_stats(nl)
-    return "k_screen+k_tersoff_sorted" if long_rows * 256 > n else "k_tersoff_atom"
+    # md_nve_run asks for no virial: the register path is the 128-register lean kernel (tersoff.cu, launch())
+    return "k_screen+k_tersoff_hot" if long_rows * 256 > n else "k_tersoff_lean"
 
 
 def measure_nve(gpu, md, cfg_index, steps, warmup, fp32, peaks, fp64_peak, with_e2e, sampler=None):
@@ -521,7 +523,7 @@ def main_ours(args):
                 "what": f"md_nve_run_host: pinned host x,v -> device, {steps} steps, x,v,f,pe -> host"},
         "gpu_launches": int(sum(r["launches"].values())),
         "roofline": {"bound": "alu", "kernel": r["kernel"], "achieved": r["alu"]["achieved"], "peak": fp64_peak,
-                     "unit": "TFLOP/s", "frac": r["alu"]["frac"], "traffic": traffic_from_profiles(r["kernel"]),
+                     "unit": "TFLOP/s", "frac": r["alu"]["frac"], "traffic": traffic_from_profiles(r["kernel"]) if n == 512000 else None,
                      "peak_source": "md_probe_fp64_peak (measured DFMA rate, this run); nominal "
                                     f"{FP64_NOMINAL_TFLOPS:.1f}",
                      "flop_equiv_per_atom": r["alu"]["flop_equiv_per_atom"], "kernel_ms": r["pair_ms"],

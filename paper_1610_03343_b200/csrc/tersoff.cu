@@ -34,6 +34,9 @@ template <class T, int NT> struct TersoffTab { TsCenter<T> c[NT]; TsPair<T> p[NT
 #ifndef LEAN_DEBUG_SLOW
 #define LEAN_DEBUG_SLOW false
 #endif
+#ifndef MD_TERSOFF_LEAN_BT
+#define MD_TERSOFF_LEAN_BT 128
+#endif
 #ifndef MD_TERSOFF_LEAN_MAXREG
 #define MD_TERSOFF_LEAN_MAXREG 128   // 4 CTAs of 128 threads per SM
 #endif
@@ -1015,8 +1018,9 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     }
     nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
     if (!virial) {                                           // NVE loop and force-only calls: the lean body
-        MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, 128, MD_TERSOFF_LEAN_MAXREG>, dim3((unsigned)((n + 127) / 128)),
-                                  dim3(128), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
+        constexpr int LBT = MD_TERSOFF_LEAN_BT;
+        MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG>, dim3((unsigned)((n + LBT - 1) / LBT)),
+                                  dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
                                   nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, nl->d_status));
         return MD_OK;
     }
