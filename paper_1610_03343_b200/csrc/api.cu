@@ -19,6 +19,9 @@ void free_all(md_neighbors* nl) {
     if (nl->h_npt) cudaFreeHost(nl->h_npt);
     if (nl->h_maxrow) cudaFreeHost(nl->h_maxrow);
     if (nl->ev_list) cudaEventDestroy(nl->ev_list);
+    if (nl->ev_fork) cudaEventDestroy(nl->ev_fork);
+    if (nl->ev_join) cudaEventDestroy(nl->ev_join);
+    if (nl->s_copy) cudaStreamDestroy(nl->s_copy);
     if (nl->ev_pool) for (cudaEvent_t e : *nl->ev_pool) cudaEventDestroy(e);
     delete nl->ev_pool; delete nl->ev_kind;
 }
@@ -283,10 +286,11 @@ int md_velocity_verlet_step(int phase, int64_t n, double* x, double* y, double* 
     return md_launch_vv(nullptr, phase, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, (cudaStream_t)stream);
 }
 
-int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+// v_ready (may be null): an event the stream waits for before the first kernel that reads the velocities
+static int nve_run_impl(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                double* x, double* y, double* z, double* vx, double* vy, double* vz,
                double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
-               int first_step, int nsteps, int rebuild_every, double r_list, void* stream) {
+               int first_step, int nsteps, int rebuild_every, double r_list, void* stream, cudaEvent_t v_ready) {
     if (!nl || !params || n < 0 || n > nl->n_cap || !valid_box(box) || nsteps < 0 || rebuild_every < 1 ||
         first_step < 0)
         return MD_ERR_ARG;
@@ -306,6 +310,7 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  pe, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
     }
+    if (v_ready) MD_CUDA_TRY(cudaStreamWaitEvent(s, v_ready, 0));
     if (nsteps == 0) return MD_OK;
     // Step s = kick+drift, [rebuild], force, kick.  The kick that ends step s and the kick+drift that
     // starts step s+1 are fused into the gather kernel of step s (gather.cu, k_gather_vv): per step the
@@ -325,6 +330,14 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
                                  last ? pe : nullptr, f, nullptr, nullptr, &vv, s)) != MD_OK) return rc;
     }
     return MD_OK;
+}
+
+int md_nve_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
+               double* x, double* y, double* z, double* vx, double* vy, double* vz,
+               double* f, int f_valid, double* pe, const double box[3], double mass_amu, double dt_fs,
+               int first_step, int nsteps, int rebuild_every, double r_list, void* stream) {
+    return nve_run_impl(nl, potential, params, precision, n, x, y, z, vx, vy, vz, f, f_valid, pe, box, mass_amu, dt_fs,
+                        first_step, nsteps, rebuild_every, r_list, stream, nullptr);
 }
 
 int md_npt_run(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
@@ -464,10 +477,23 @@ int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int pre
     double* d = nl->e2e;
     double* host_in[6] = {x, y, z, vx, vy, vz};
     const size_t bytes = sizeof(double) * (size_t)n;
-    for (int a = 0; a < 6; ++a)
+    if (!nl->s_copy) {
+        if (cudaStreamCreateWithFlags(&nl->s_copy, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&nl->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&nl->ev_join, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+    }
+    // positions on the caller's stream; velocities on the copy stream (after whatever `s` still does with the
+    // buffers), joined just before the first kick: list build and first force evaluation overlap with them
+    MD_CUDA_TRY(cudaEventRecord(nl->ev_fork, s));
+    MD_CUDA_TRY(cudaStreamWaitEvent(nl->s_copy, nl->ev_fork, 0));
+    for (int a = 0; a < 3; ++a)
         MD_CUDA_TRY(cudaMemcpyAsync(d + a * n, host_in[a], bytes, cudaMemcpyHostToDevice, s));
-    int rc = md_nve_run(nl, potential, params, precision, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n,
-                        d + 6 * n, 0, d + 9 * n, box, mass_amu, dt_fs, 0, nsteps, rebuild_every, r_list, stream);
+    for (int a = 3; a < 6; ++a)
+        MD_CUDA_TRY(cudaMemcpyAsync(d + a * n, host_in[a], bytes, cudaMemcpyHostToDevice, nl->s_copy));
+    MD_CUDA_TRY(cudaEventRecord(nl->ev_join, nl->s_copy));
+    int rc = nve_run_impl(nl, potential, params, precision, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n,
+                          d + 6 * n, 0, d + 9 * n, box, mass_amu, dt_fs, 0, nsteps, rebuild_every, r_list, stream,
+                          nl->ev_join);
     if (rc != MD_OK) return rc;
     for (int a = 0; a < 6; ++a)
         MD_CUDA_TRY(cudaMemcpyAsync(host_in[a], d + a * n, bytes, cudaMemcpyDeviceToHost, s));

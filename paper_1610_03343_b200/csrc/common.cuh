@@ -68,6 +68,9 @@ struct md_neighbors {
     double ms_acc[MD_N_KINDS];
     // Berendsen NPT (md_npt_run): per-atom virial [9][n], reduction scratch, pinned landing zone
     double* npt_w; int64_t npt_cap; double* npt_part; double* h_npt;
+    // md_nve_run_host: the velocities travel on a second stream while the list build and the first force
+    // evaluation (which need positions only) already run
+    cudaStream_t s_copy; cudaEvent_t ev_fork, ev_join;
     // e2e device state (md_nve_run_host)
     double* e2e;            // [13][n] x,y,z,vx,vy,vz,f[3],pe + spare
     int64_t e2e_cap;
