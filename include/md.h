@@ -26,8 +26,8 @@
  *     max_neighbors, a missing reverse entry, too many in-range neighbours) latch a status word in
  *     the handle; md_neighbors_status() synchronises the stream and returns it.
  *   - Capacity limits beyond max_neighbors (all latch MD_ERR_NEIGHBOR_OVERFLOW, results are then invalid):
- *     at most 32 neighbours of one atom inside the force range; the register Tersoff kernel's per-thread
- *     fallback for rows longer than 4 holds 16 in-range neighbours; the sorted kernels keep the in-range
+ *     at most 32 neighbours of one atom inside the force range (also the limit of the warp-per-atom general
+ *     path that the register Tersoff kernels use for rows longer than 4); the sorted kernels keep the in-range
  *     neighbours of a 128-atom tile in a shared-memory pool of 128 x 8 (Tersoff) or 128 x 12
  *     (Stillinger-Weber) slots, of which each of the tile's four warps (atoms sorted by in-range count) takes
  *     32 x its largest count: the four largest-per-warp counts must sum to <= 32 (Tersoff) / 48 (SW).
@@ -78,8 +78,8 @@ int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream);
 
 /* Row statistics of the current list (HOST ints, either may be NULL): the longest row and the number
  * of rows longer than 4 entries.  Waits for the last build / import on its stream to finish.  The
- * Tersoff call uses them to choose its kernel: the register kernel (k_tersoff_atom) while at most one
- * row in 256 is longer than 4, else the lanes = pairs kernel (k_tersoff_pairs_cta). */
+ * Tersoff call uses them to choose its kernel: the register kernels (k_tersoff_lean without, k_tersoff_atom
+ * with a virial output) while at most one row in 256 is longer than 4, else k_screen + k_tersoff_hot. */
 int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than_4);
 
 /* Copy the current list out / in (DEVICE int32 buffers): NN[n]; NL[max_neighbors][n] neighbour-major,

@@ -23,8 +23,9 @@ __device__ __forceinline__ void store_rec(PairRec64* q, double px, double py, do
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(q), "d"(px), "d"(py), "d"(pz), "d"(0.0) : "memory");
 }
 // The same record as two 128-bit stores, for code inside a non-inlined device function: ptxas 12.9 turned the
-// 256-bit store above into a single 64-bit one (only Px reached memory) when tersoff_pair_generic was compiled
-// as a callee of the 128-register kernel k_tersoff_lean (seen in the SASS and as stale records on the GPU).
+// 256-bit store above into a single 64-bit one (only Px reached memory) when the per-thread general path of round 1
+// was compiled as a callee of the 128-register kernel k_tersoff_lean (seen in the SASS and as stale records on
+// the GPU).  tersoff_warp_atom, today's non-inlined callee, uses this form.
 __device__ __forceinline__ void store_rec_2x128(PairRec64* q, double px, double py, double pz) {
     double2* d = reinterpret_cast<double2*>(q);
     d[0] = make_double2(px, py);
