@@ -31,6 +31,8 @@ __device__ __forceinline__ int cell_coord(double c, double inv, int nc) {
 __global__ void k_bin(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                       const double* __restrict__ z, Grid g, int32_t* __restrict__ cell_of,
                       int32_t* __restrict__ rank, int32_t* __restrict__ cell_count) {
+    md_grid_wait();                                          // chained build kernels: see md_launch_build
+    md_grid_release();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int cx = cell_coord(x[i], g.inv_cell[0], g.nc[0]);
@@ -75,6 +77,8 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int* total, int* warp
 }
 
 __global__ void k_scan_local(int32_t* __restrict__ data, int64_t n, int32_t* __restrict__ tile_sums) {
+    md_grid_wait();                                          // chained build kernels: see md_launch_build
+    md_grid_release();
     __shared__ int warp_sums[32];
     const int64_t base = ((int64_t)blockIdx.x * SCAN_BT + threadIdx.x) * SCAN_IT;
     int v[SCAN_IT];
@@ -95,6 +99,8 @@ __global__ void k_scan_local(int32_t* __restrict__ data, int64_t n, int32_t* __r
 }
 
 __global__ void k_scan_tiles(int32_t* __restrict__ tile_sums, int ntiles) {
+    md_grid_wait();                                          // chained build kernels: see md_launch_build
+    md_grid_release();
     __shared__ int warp_sums[32];
     int carry = 0;
     for (int b = 0; b < ntiles; b += blockDim.x) {
@@ -109,6 +115,8 @@ __global__ void k_scan_tiles(int32_t* __restrict__ tile_sums, int ntiles) {
 
 __global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t* __restrict__ tile_sums,
                            int32_t grand_total) {
+    md_grid_wait();                                          // chained build kernels: see md_launch_build
+    md_grid_release();
     const int64_t base = ((int64_t)blockIdx.x * SCAN_BT + threadIdx.x) * SCAN_IT;
     const int add = tile_sums[blockIdx.x];
 #pragma unroll
@@ -121,6 +129,8 @@ __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double*
                           const double* __restrict__ z, const int32_t* __restrict__ cell_of,
                           const int32_t* __restrict__ rank, const int32_t* __restrict__ cell_start,
                           double4* __restrict__ sorted, float4* __restrict__ sortedf) {
+    md_grid_wait();                                          // chained build kernels: see md_launch_build
+    md_grid_release();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int pos = cell_start[cell_of[i]] + rank[i];
@@ -138,6 +148,8 @@ __global__ void __launch_bounds__(SEARCH_BT)
 k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __restrict__ sortedf,
          const int32_t* __restrict__ cell_start, int K, float rc2_lo, float rc2_hi, int32_t* __restrict__ NN,
          int32_t* __restrict__ NL, int* __restrict__ status) {
+    md_grid_wait();
+    md_grid_release();
     extern __shared__ int s_nb[];                            // [K][SEARCH_BT]: this thread's row, sorted
     const int tid = threadIdx.x;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + tid;
@@ -252,6 +264,8 @@ template <bool CHECK>
 __global__ void __launch_bounds__(128)
 k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
           uint8_t* __restrict__ REV, int* __restrict__ status) {
+    md_grid_wait();
+    md_grid_release();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int nn = min(NN[i], K);
@@ -328,8 +342,10 @@ int md_launch_reverse(md_neighbors* nl, cudaStream_t s, int check) {
     const int64_t n = nl->n;
     if (n == 0) return MD_OK;
     ProfScope prof(nl, MD_KIND_BUILD, 1, s);
+    // after k_search (a build) as a programmatic dependent; after the copies of an import as a normal launch
     if (check) k_reverse<true><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
-    else k_reverse<false><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
+    else MD_CUDA_TRY(md_launch_pdl(k_reverse<false>, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, s, true, n, nl->K, nl->NN,
+                                   nl->NL, nl->REV, nl->d_status));
     MD_CUDA_TRY(cudaGetLastError());
     MD_CUDA_TRY(cudaMemcpyAsync(nl->h_maxrow, nl->d_status + 1, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     MD_CUDA_TRY(cudaEventRecord(nl->ev_list, s));
@@ -368,12 +384,15 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     {
     ProfScope prof(nl, MD_KIND_BUILD, 6, s);
     MD_CUDA_TRY(cudaMemsetAsync(nl->cell_count, 0, sizeof(int32_t) * (ncell + 1), s));
+    // The seven kernels of a build each need everything the one before wrote, so each starts with
+    // griddepcontrol.wait and is launched as a programmatic dependent: only the launch latency and ramp of the
+    // next kernel overlap with the drain of the previous one (k_bin follows a memset and is launched normally).
     k_bin<<<gb, 256, 0, s>>>(n, x, y, z, g, nl->cell_of, nl->rank_in_cell, nl->cell_count);
-    k_scan_local<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks);
-    k_scan_tiles<<<1, 1024, 0, s>>>(nl->scan_blocks, ntiles);
-    k_scan_add<<<ntiles, SCAN_BT, 0, s>>>(nl->cell_count, ncell, nl->scan_blocks, (int32_t)n);
-    k_scatter<<<gb, 256, 0, s>>>(n, x, y, z, nl->cell_of, nl->rank_in_cell, nl->cell_count, nl->sorted,
-                                 nl->sortedf);
+    MD_CUDA_TRY(md_launch_pdl(k_scan_local, dim3(ntiles), dim3(SCAN_BT), 0, s, true, nl->cell_count, ncell, nl->scan_blocks));
+    MD_CUDA_TRY(md_launch_pdl(k_scan_tiles, dim3(1), dim3(1024), 0, s, true, nl->scan_blocks, ntiles));
+    MD_CUDA_TRY(md_launch_pdl(k_scan_add, dim3(ntiles), dim3(SCAN_BT), 0, s, true, nl->cell_count, ncell, nl->scan_blocks, (int32_t)n));
+    MD_CUDA_TRY(md_launch_pdl(k_scatter, dim3(gb), dim3(256), 0, s, true, n, x, y, z, nl->cell_of, nl->rank_in_cell,
+                              nl->cell_count, nl->sorted, nl->sortedf));
     // FP32 screen.  A coordinate in [0, L) rounds to float within u = 2^-24 Lmax; the shifted reference
     // x +- L carries at most 4u, so each float component differs from the canonical FP64 one by less than
     // 5u (+ 1e-13 of FP64 rounding), and for a candidate near the cut-off |d2_f32 - d2| is below
@@ -384,8 +403,9 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     const double e = 6.0 * Lmax * 5.9604645e-8;
     const double band = 32.0 * (r_list + e) * e + 1e-6 * g.rc2;
     const float rc2_lo = (float)(g.rc2 - band) , rc2_hi = (float)(g.rc2 + band);
-    k_search<<<(unsigned)((n + SEARCH_BT - 1) / SEARCH_BT), SEARCH_BT, sizeof(int) * SEARCH_BT * nl->K, s>>>(
-        n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K, rc2_lo, rc2_hi, nl->NN, nl->NL, nl->d_status);
+    MD_CUDA_TRY(md_launch_pdl(k_search, dim3((unsigned)((n + SEARCH_BT - 1) / SEARCH_BT)), dim3(SEARCH_BT),
+                              sizeof(int) * SEARCH_BT * nl->K, s, true, n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K,
+                              rc2_lo, rc2_hi, nl->NN, nl->NL, nl->d_status));
     }
     MD_CUDA_TRY(cudaGetLastError());
     return md_launch_reverse(nl, s, 0);
