@@ -139,12 +139,28 @@ __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double*
     sortedf[pos] = make_float4((float)xi, (float)yi, (float)zi, __int_as_float((int)i));
 }
 
+// The canonical FP64 predicate of reading A7 (explicit roundings, no contraction), evaluated only for a candidate
+// whose FP32 distance falls inside the undecided band (about one in 10^4).  Not inlined: the search loop is
+// instantiated 36 times, and with this block inside each copy the kernel outgrew the instruction cache
+// (14 % of its stall samples were "no instruction").
+__device__ __noinline__ bool search_decide_fp64(const double4* __restrict__ sorted, int q, double ax, double ay, double az,
+                                                double Lx, double Ly, double Lz, double rc2) {
+    const double4 b = sorted[q];
+    const double dx = md_min_image(__dsub_rn(b.x, ax), Lx, 0.5 * Lx);
+    const double dy = md_min_image(__dsub_rn(b.y, ay), Ly, 0.5 * Ly);
+    const double dz = md_min_image(__dsub_rn(b.z, az), Lz, 0.5 * Lz);
+    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < rc2;
+}
+
 constexpr int SEARCH_BT = 128;
 #ifndef SEARCH_UNROLL
 #define SEARCH_UNROLL 2
 #endif
 
-__global__ void __launch_bounds__(SEARCH_BT)
+#ifndef SEARCH_MIN_CTAS
+#define SEARCH_MIN_CTAS 8
+#endif
+__global__ void __launch_bounds__(SEARCH_BT, SEARCH_MIN_CTAS)
 k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __restrict__ sortedf,
          const int32_t* __restrict__ cell_start, int K, float rc2_lo, float rc2_hi, int32_t* __restrict__ NN,
          int32_t* __restrict__ NL, int* __restrict__ status) {
@@ -173,14 +189,7 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
         const float d2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
         const int j = __float_as_int(bf.w);
         bool hit = d2f < rc2_hi && j != i;
-        if (hit && d2f >= rc2_lo) {
-            const double4 b = sorted[q];
-            const double dx = md_min_image(__dsub_rn(b.x, a.x), g.L[0], g.halfL[0]);
-            const double dy = md_min_image(__dsub_rn(b.y, a.y), g.L[1], g.halfL[1]);
-            const double dz = md_min_image(__dsub_rn(b.z, a.z), g.L[2], g.halfL[2]);
-            const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-            hit = d2 < g.rc2;
-        }
+        if (hit && d2f >= rc2_lo) hit = search_decide_fp64(sorted, q, a.x, a.y, a.z, g.L[0], g.L[1], g.L[2], g.rc2);
         if (hit && cnt < K) s_nb[cnt * SEARCH_BT + tid] = j;
         cnt += hit ? 1 : 0;
     };
