@@ -139,19 +139,6 @@ __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double*
     sortedf[pos] = make_float4((float)xi, (float)yi, (float)zi, __int_as_float((int)i));
 }
 
-// The canonical FP64 predicate of reading A7 (explicit roundings, no contraction), evaluated only for a candidate
-// whose FP32 distance falls inside the undecided band (about one in 10^4).  Not inlined: the search loop is
-// instantiated 36 times, and with this block inside each copy the kernel outgrew the instruction cache
-// (14 % of its stall samples were "no instruction").
-__device__ __noinline__ bool search_decide_fp64(const double4* __restrict__ sorted, int q, double ax, double ay, double az,
-                                                double Lx, double Ly, double Lz, double rc2) {
-    const double4 b = sorted[q];
-    const double dx = md_min_image(__dsub_rn(b.x, ax), Lx, 0.5 * Lx);
-    const double dy = md_min_image(__dsub_rn(b.y, ay), Ly, 0.5 * Ly);
-    const double dz = md_min_image(__dsub_rn(b.z, az), Lz, 0.5 * Lz);
-    return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < rc2;
-}
-
 constexpr int SEARCH_BT = 128;
 #ifndef SEARCH_UNROLL
 #define SEARCH_UNROLL 2
@@ -166,7 +153,7 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
          int32_t* __restrict__ NL, int* __restrict__ status) {
     md_grid_wait();
     md_grid_release();
-    extern __shared__ int s_nb[];                            // [K][SEARCH_BT]: this thread's row, sorted
+    extern __shared__ int s_nb[];                            // [K + 1][SEARCH_BT]: this thread's row (+ a scratch slot)
     const int tid = threadIdx.x;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + tid;
     if (t >= n) return;
@@ -179,18 +166,21 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
     const float Lxf = (float)g.L[0], Lyf = (float)g.L[1], Lzf = (float)g.L[2];
     int cnt = 0;
 
-    // One candidate.  The FP32 distance decides whenever it is outside the band [rc2_lo, rc2_hi) that its
-    // error bound leaves open (see md_launch_build); inside the band (about one candidate in 10^4) the
-    // canonical FP64 predicate of reading A7 decides, with explicit roundings and no contraction.  Either
-    // way the outcome is that predicate's.  A hit is appended with a predicated store (no divergent
-    // insertion inside the scan); the row is sorted once at the end.
+    // One candidate, branch-free.  The FP32 distance decides whenever it is outside the band [rc2_lo, rc2_hi)
+    // that its error bound leaves open (see md_launch_build).  A candidate below rc2_hi is a provisional hit; one
+    // inside the band (about one candidate in 10^4) only marks the row as `unc`ertain, and such a row is checked
+    // entry by entry with the canonical FP64 predicate of reading A7 after the scan, so the outcome is always that
+    // predicate's.  The candidate's cell-order position is written to the row's next slot unconditionally and
+    // the slot advances only on a hit (no branch, no reconvergence point in the loop: the branchy version spent
+    // ~35 instructions per candidate, this one ~16).
+    unsigned unc = 0u;
+    const int Kslot = K;                                     // row slot K is a scratch slot: entries 0..K-1 stay valid on overflow
     auto test = [&](int q, const float4 bf, float xs, float ys, float zs) {
         const float fx = bf.x - xs, fy = bf.y - ys, fz = bf.z - zs;
         const float d2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
-        const int j = __float_as_int(bf.w);
-        bool hit = d2f < rc2_hi && j != i;
-        if (hit && d2f >= rc2_lo) hit = search_decide_fp64(sorted, q, a.x, a.y, a.z, g.L[0], g.L[1], g.L[2], g.rc2);
-        if (hit && cnt < K) s_nb[cnt * SEARCH_BT + tid] = j;
+        const bool hit = d2f < rc2_hi && __float_as_int(bf.w) != i;
+        unc |= (hit && d2f >= rc2_lo) ? 1u : 0u;
+        s_nb[min(cnt, Kslot) * SEARCH_BT + tid] = q;
         cnt += hit ? 1 : 0;
     };
     // a contiguous range of the cell-ordered array, SEARCH_UNROLL candidates in flight at a time
@@ -243,12 +233,28 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
 #pragma unroll
         for (int c = 0; c < 9; ++c) scan(beg[c], end[c], xss[c / 3], yss[c % 3], zs);
     }
+    if (cnt > K) { atomicOr(&status[0], MD_DEV_ROW_OVERFLOW); cnt = K; }   // counted before the check below: conservative
+    {   // cell-order position -> atom index; rows marked uncertain keep only what the FP64 predicate confirms
+        int out = 0;
+        for (int m = 0; m < cnt; ++m) {
+            const int q = s_nb[m * SEARCH_BT + tid];
+            const double4 b = sorted[q];
+            bool ok = true;
+            if (unc) {
+                const double dx = md_min_image(__dsub_rn(b.x, a.x), g.L[0], g.halfL[0]);
+                const double dy = md_min_image(__dsub_rn(b.y, a.y), g.L[1], g.halfL[1]);
+                const double dz = md_min_image(__dsub_rn(b.z, a.z), g.L[2], g.halfL[2]);
+                ok = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx))) < g.rc2;
+            }
+            if (ok) s_nb[out++ * SEARCH_BT + tid] = (int)__double_as_longlong(b.w);
+        }
+        cnt = out;
+    }
     {   // longest row: one atomic per warp
         const unsigned act = __activemask();
         const int wmax = __reduce_max_sync(act, cnt);
         if ((tid & 31) == __ffs(act) - 1) atomicMax(&status[1], wmax);
     }
-    if (cnt > K) { atomicOr(&status[0], MD_DEV_ROW_OVERFLOW); cnt = K; }
     NN[i] = cnt;
     for (int m = 1; m < cnt; ++m) {                          // insertion sort of the (short) row by index
         const int j = s_nb[m * SEARCH_BT + tid];
@@ -413,7 +419,7 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     const double band = 32.0 * (r_list + e) * e + 1e-6 * g.rc2;
     const float rc2_lo = (float)(g.rc2 - band) , rc2_hi = (float)(g.rc2 + band);
     MD_CUDA_TRY(md_launch_pdl(k_search, dim3((unsigned)((n + SEARCH_BT - 1) / SEARCH_BT)), dim3(SEARCH_BT),
-                              sizeof(int) * SEARCH_BT * nl->K, s, true, n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K,
+                              sizeof(int) * SEARCH_BT * (nl->K + 1), s, true, n, g, nl->sorted, nl->sortedf, nl->cell_count, nl->K,
                               rc2_lo, rc2_hi, nl->NN, nl->NL, nl->d_status));
     }
     MD_CUDA_TRY(cudaGetLastError());
