@@ -153,7 +153,7 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->Q, n * K * sizeof(PairRec64)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->MASK, n * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->bin_list, 3 * n * sizeof(int32_t)) == cudaSuccess;
-    ok = ok && cudaMalloc(&nl->bin_count, 4 * sizeof(int32_t)) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->bin_count, 8 * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->cell_of, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->rank_in_cell, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->sorted, n * sizeof(double4)) == cudaSuccess;
@@ -163,6 +163,7 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaEventCreateWithFlags(&nl->ev_list, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { cudaGetLastError(); free_all(nl); delete nl; return MD_ERR_ALLOC; }
     cudaMemset(nl->d_status, 0, 3 * sizeof(int));
+    cudaMemset(nl->bin_count, 0, 8 * sizeof(int32_t));
     *out = nl;
     return MD_OK;
 }

@@ -38,7 +38,11 @@ struct md_neighbors {
     void* Q;                // K*n*32 bytes
     unsigned long long* MASK;  // [n] bit m set <=> slot m is inside the force range
     int32_t* bin_list;      // [3][n] atom indices by in-range-count bin (pair_sort.cuh, Bins), written by k_screen
-    int32_t* bin_count;     // [3]
+    int32_t* bin_count;     // [2][4] two sets used alternately (bin_phase), each zeroed by the launch before its use
+    int bin_phase;
+    int gather_pdl;         // the last pair launch wants the fused gather as its programmatic dependent (measured per
+                            // path: +3 % after k_tersoff_lean, 0 after k_sw_sorted, -6 % after k_tersoff_hot, whose 148
+                            // long-running tail CTAs then share their SMs with early-resident gather CTAs)
     int q_dense;            // layout of the records the last pair kernel wrote: 1 = slot counts in-range entries
                             // (sorted kernels, MASK known beforehand), 0 = slot is the list position
     // cell structures

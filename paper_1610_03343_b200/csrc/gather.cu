@@ -138,7 +138,7 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
 #define MD_GATHER_VV(TT, RR, MODE)                                                                        \
-    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, true, n, nl->K, (const RR*)nl->Q,            \
+    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, nl->gather_pdl != 0, n, nl->K, (const RR*)nl->Q,            \
                               nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z, vv->vx, vv->vy, vv->vz, vv->hk, vv->dt,    \
                               box[0], box[1], box[2]))
         if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }

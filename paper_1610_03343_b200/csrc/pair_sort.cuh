@@ -84,8 +84,8 @@ template <class T> struct RangeTab { int nt; T r2[16]; };
 
 template <class T, int U>
 __device__ __forceinline__ unsigned long long
-screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const double* __restrict__ y,
-           const double* __restrict__ z, const MinImage& mi, const int32_t* __restrict__ NL,
+screen_row(unsigned i, unsigned n, int nn, const double* x, const double* y, const double* z,   // plain loads: see k_screen
+           const MinImage& mi, const int32_t* __restrict__ NL,
            const RangeTab<T>& rt, const int32_t* __restrict__ types) {
     const int trow = types ? types[i] * rt.nt : 0;
     const double xi = x[i], yi = y[i], zi = z[i];
@@ -138,19 +138,27 @@ screen_row(unsigned i, unsigned n, int nn, const double* __restrict__ x, const d
 struct Bins {
     int b0, b1;
     int32_t* list;      // [3][n]
-    int32_t* count;     // [3], zeroed before the screen
+    int32_t* count;     // [4] of this launch: zero on entry
+    int32_t* count_next;// [4] of the next launch (the other half of a ping-pong pair): zeroed by this one, whose
+                        // wait has seen the last reader of that half finish -- no memset between the kernels
 };
 
 template <class T>
 __global__ void __launch_bounds__(256, 4)
-k_screen(unsigned n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+k_screen(unsigned n, const double* x, const double* y, const double* z,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
          RangeTab<T> rt, const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK, Bins bins) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     int bin = -1;
+    // Inside md_nve_run: a programmatic dependent of the fused gather that wrote x, y, z (common.cuh,
+    // md_launch_pdl); the row length is requested while that kernel drains, the coordinates are read after the
+    // wait through plain (non-.nc) loads.
+    int nn = i < n ? NN[i] : 0;
+    md_grid_wait();
+    md_grid_release();
+    if (bins.count_next && i < 4) bins.count_next[i] = 0;
     if (i < n) {
         const MinImage mi = make_min_image(Lx, Ly, Lz);
-        int nn = NN[i];
         if (nn > 64) nn = 64;
         const unsigned long long mask = screen_row<T, 4>(i, n, nn, x, y, z, mi, NL, rt, types);
         MASK[i] = mask;
@@ -193,9 +201,9 @@ __device__ __forceinline__ int ld_early(const uint8_t* p) {
     asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ unsigned long long ld_early(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.global.nc.u64 %0, [%1];" : "=l"(v) : "l"(p));
+__device__ __forceinline__ unsigned long long ld_early(const unsigned long long* p) {   // MASK: written by the kernel
+    unsigned long long v;                                                               // before (k_screen): no .nc
+    asm volatile("ld.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
     return v;
 }
 

@@ -67,7 +67,7 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
             const double* __restrict__ z, double Lx, double Ly, double Lz,
             const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
             const uint8_t* __restrict__ REV, SWDev<T> p, const double* __restrict__ gtab,
-            Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+            Rec* __restrict__ Q, const unsigned long long* MASK,    // MASK: k_screen, the kernel before, wrote it
             double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
             int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -75,6 +75,8 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
     const int tid = threadIdx.x, lane = tid & 31;
     const int64_t A0 = (int64_t)blockIdx.x * BT;
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);       // visible after the sort's barriers
+    md_grid_wait();                                          // programmatic dependent of k_screen (common.cuh)
+    md_grid_release();
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
 
     // in-range masks of the tile (k_screen wrote them), tile order
@@ -273,7 +275,8 @@ k_sw_sorted(int64_t n, const double* __restrict__ x, const double* __restrict__ 
 
 template <class T, class Rec>
 int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
-           const double box[3], const md_sw_params* hp, double* pe, double* f, double* virial, cudaStream_t s) {
+           const double box[3], const md_sw_params* hp, double* pe, double* f, double* virial, bool pdl,
+           cudaStream_t s) {
     SWDev<T> p;
     const double rc = hp->a * hp->sigma;
     p.Aeps = (T)(hp->A * hp->epsilon); p.B = (T)hp->B; p.sigma = (T)hp->sigma;
@@ -281,11 +284,13 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     p.leps = (T)(hp->lambda * hp->epsilon); p.cos0 = (T)hp->cos0; p.p = (T)hp->p; p.q = (T)hp->q;
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
+    nl->gather_pdl = 0;
     ProfScope prof(nl, MD_KIND_PAIR, 2, s);
     ps::RangeTab<T> rt;
     rt.nt = 1; rt.r2[0] = p.rc2;
-    ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2], nl->NN,
-                                                                 nl->NL, rt, nullptr, nl->MASK, ps::Bins{0, 0, nullptr, nullptr});
+    MD_CUDA_TRY(md_launch_pdl(ps::k_screen<T>, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, s, pdl, (unsigned)n, x, y, z,
+                              box[0], box[1], box[2], nl->NN, nl->NL, rt, (const int32_t*)nullptr, nl->MASK,
+                              ps::Bins{0, 0, nullptr, nullptr, nullptr}));
     nl->q_dense = 1;
     constexpr int BT = 128, PCA = MD_SW_POOL_PER_ATOM;
     using Sm = SWSmem<T, BT, PCA>;
@@ -294,10 +299,9 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
                                                    : k_sw_sorted<T, Rec, BT, PCA, -1, -1, MD_SW_MAXREG>;
     const int rcs = md_allow_dynamic_smem((const void*)kern, (int)sizeof(Sm));
     if (rcs != MD_OK) return rcs;
-    kern<<<(unsigned)((n + BT - 1) / BT), BT, sizeof(Sm), s>>>(
-        n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK,
-        pe, f, virial, nl->d_status);
-    MD_CUDA_TRY(cudaGetLastError());
+    MD_CUDA_TRY(md_launch_pdl(kern, dim3((unsigned)((n + BT - 1) / BT)), dim3(BT), sizeof(Sm), s, true, n, x, y, z, box[0],
+                              box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab, (Rec*)nl->Q,
+                              (const unsigned long long*)nl->MASK, pe, f, virial, nl->d_status));
     return MD_OK;
 }
 
@@ -308,8 +312,9 @@ int md_launch_sw(md_neighbors* nl, int64_t n, const double* x, const double* y, 
                  const md_sw_params* p, int precision, double* pe, double* f, double* virial,
                  double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0) return MD_OK;
-    int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, s)
-                                  : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, s);
+    const bool pdl = vv && vv->pdl_pair;                     // the list is unchanged and the kernel before is the loop's own
+    int rc = precision == MD_FP32 ? launch<float, float4>(nl, n, x, y, z, box, p, pe, f, virial, pdl, s)
+                                  : launch<double, PairRec64>(nl, n, x, y, z, box, p, pe, f, virial, pdl, s);
     if (rc != MD_OK) return rc;
     return md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, f, virial, heat, vv, s);
 }

@@ -636,8 +636,8 @@ __device__ __forceinline__ void
 tersoff_binned_cta(int64_t cta, int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                    const double* __restrict__ z, double Lx, double Ly, double Lz,
                    const int32_t* __restrict__ NL, const uint8_t* __restrict__ REV,
-                   const int32_t* __restrict__ list, const int32_t* __restrict__ count, const TersoffDev<T>& p,
-                   const fm::Tab& tb, Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                   const int32_t* list, const int32_t* count, const TersoffDev<T>& p,
+                   const fm::Tab& tb, Rec* __restrict__ Q, const unsigned long long* MASK,
                    double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial) {
     const int64_t cnt = *count;
     const int64_t t0 = cta * BT + threadIdx.x;
@@ -704,9 +704,9 @@ tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, 
                     const double* __restrict__ z, double Lx, double Ly, double Lz,
                     const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                     const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const TersoffTab<T, NT>& tab,
-                    const int32_t* __restrict__ types, const int32_t* __restrict__ list,
-                    const int32_t* __restrict__ count,
-                    Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                    const int32_t* __restrict__ types, const int32_t* list,
+                    const int32_t* count,
+                    Rec* __restrict__ Q, const unsigned long long* MASK,
                     double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                     int* __restrict__ status) {
     const int tid = threadIdx.x, lane = tid & 31;
@@ -876,14 +876,16 @@ k_tersoff_sorted(int64_t n, const double* __restrict__ x, const double* __restri
                  const double* __restrict__ z, double Lx, double Ly, double Lz,
                  const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                  const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, NT> tab,
-                 const int32_t* __restrict__ types, const int32_t* __restrict__ list,
-                 const int32_t* __restrict__ count, const double* __restrict__ gtab,
-                 Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+                 const int32_t* __restrict__ types, const int32_t* list,
+                 const int32_t* count, const double* __restrict__ gtab,
+                 Rec* __restrict__ Q, const unsigned long long* MASK,
                  double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
                  int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);
+    md_grid_wait();                                          // programmatic dependent of k_screen, which wrote MASK and
+    md_grid_release();                                       // the bin lists (read below through plain loads)
     __syncthreads();
     tersoff_sorted_ctas<T, Rec, BT, PCA, NT>(blockIdx.x, gridDim.x, s, tb, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tab,
                                              types, list, count, Q, MASK, pe, f, virial, status);
@@ -900,13 +902,15 @@ k_tersoff_hot(int64_t n, int tail_ctas, const double* __restrict__ x, const doub
               const double* __restrict__ z, double Lx, double Ly, double Lz,
               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
               const uint8_t* __restrict__ REV, TersoffDev<T> p, TersoffTab<T, 1> tab,
-              const int32_t* __restrict__ lists, const int32_t* __restrict__ counts,
-              const double* __restrict__ gtab, Rec* __restrict__ Q, const unsigned long long* __restrict__ MASK,
+              const int32_t* lists, const int32_t* counts,
+              const double* __restrict__ gtab, Rec* __restrict__ Q, const unsigned long long* MASK,
               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
               int* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TersoffSortSmem<T, BT, PCA>& s = *reinterpret_cast<TersoffSortSmem<T, BT, PCA>*>(smem_raw);
     const fm::Tab tb = fm::stage_tables(s.tab, gtab);
+    md_grid_wait();                                          // as k_tersoff_sorted
+    md_grid_release();
     __syncthreads();
     if ((int)blockIdx.x < tail_ctas)
         tersoff_sorted_ctas<T, Rec, BT, PCA, 1>(blockIdx.x, tail_ctas, s, tb, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tab,
@@ -951,7 +955,8 @@ void make_tab(const md_tersoff_multi_params* hp, TersoffTab<T, NT>* tab, ps::Ran
 template <class T, class Rec, int NT>
 int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                   const double box[3], const TersoffDev<T>& p, const md_tersoff_multi_params* mp,
-                  const int32_t* types, const double* gtab, double* pe, double* f, double* virial, cudaStream_t s) {
+                  const int32_t* types, const double* gtab, double* pe, double* f, double* virial, bool pdl,
+                  cudaStream_t s) {
     TersoffTab<T, NT> tab;
     ps::RangeTab<T> rt;
     make_tab<T, NT>(mp, &tab, &rt);
@@ -960,11 +965,13 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
     ps::Bins bins;
     bins.b0 = 4; bins.b1 = 4;
     bins.list = NT == 1 ? nl->bin_list : nullptr;
-    bins.count = nl->bin_count;
-    if (NT == 1) MD_CUDA_TRY(cudaMemsetAsync(nl->bin_count, 0, 4 * sizeof(int32_t), s));
+    nl->bin_phase ^= 1;                                       // two sets of counters: this launch's, and the next one's
+    int32_t* const counts = nl->bin_count + 4 * nl->bin_phase;   // (zeroed by this k_screen, see pair_sort.cuh)
+    bins.count = counts;
+    bins.count_next = NT == 1 ? nl->bin_count + 4 * (nl->bin_phase ^ 1) : nullptr;
     nl->launches[MD_KIND_PAIR] += NT == 1 ? 2 : 1;
-    ps::k_screen<T><<<(unsigned)((n + 255) / 256), 256, 0, s>>>((unsigned)n, x, y, z, box[0], box[1], box[2],
-                                                                 nl->NN, nl->NL, rt, NT > 1 ? types : nullptr, nl->MASK, bins);
+    MD_CUDA_TRY(md_launch_pdl(ps::k_screen<T>, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, s, pdl, (unsigned)n, x, y, z,
+                              box[0], box[1], box[2], nl->NN, nl->NL, rt, NT > 1 ? types : (const int32_t*)nullptr, nl->MASK, bins));
     nl->q_dense = 1;
     constexpr int BT = 128, PCA = MD_TERSOFF_POOL_PER_ATOM;
     const unsigned grid = (unsigned)((n + BT - 1) / BT);      // sized for "every atom in this bin"; surplus CTAs exit at once
@@ -980,13 +987,15 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
         auto hot = k_tersoff_hot<T, Rec, 4, BT, PCA, 168>;
         const int rch = md_allow_dynamic_smem((const void*)hot, (int)sizeof(Sm));
         if (rch != MD_OK) return rch;
-        hot<<<grid + (unsigned)tail, BT, sizeof(Sm), s>>>(n, tail, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV,
-                                                        p, tab, nl->bin_list, nl->bin_count, gtab, (Rec*)nl->Q, nl->MASK,
-                                                        pe, f, virial, nl->d_status);
+        MD_CUDA_TRY(md_launch_pdl(hot, dim3(grid + (unsigned)tail), dim3(BT), sizeof(Sm), s, true, n, tail, x, y, z, box[0],
+                                  box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, (const int32_t*)nl->bin_list,
+                                  (const int32_t*)counts, gtab, (Rec*)nl->Q, (const unsigned long long*)nl->MASK, pe, f,
+                                  virial, nl->d_status));
     } else {
-        kern<<<std::min<unsigned>(grid, 3u * (unsigned)sms), BT, sizeof(Sm), s>>>(
-            n, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types, nullptr, nullptr, gtab,
-            (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status);
+        MD_CUDA_TRY(md_launch_pdl(kern, dim3(std::min<unsigned>(grid, 3u * (unsigned)sms)), dim3(BT), sizeof(Sm), s, true, n,
+                                  x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types,
+                                  (const int32_t*)nullptr, (const int32_t*)nullptr, gtab, (Rec*)nl->Q,
+                                  (const unsigned long long*)nl->MASK, pe, f, virial, nl->d_status));
     }
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
@@ -997,6 +1006,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
            const double box[3], const md_tersoff_params* hp, double* pe, double* f, double* virial,
            bool pdl, cudaStream_t s) {
     const TersoffDev<T> p = make_dev<T>(hp);
+    nl->gather_pdl = 0;
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
@@ -1014,7 +1024,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     if ((int64_t)long_rows * 256 > n) {
         md_tersoff_multi_params one;
         one.ntypes = 1; one.elem[0] = *hp; one.chi[0][0] = 1.0;
-        return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, &one, nullptr, gtab, pe, f, virial, s);
+        return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, &one, nullptr, gtab, pe, f, virial, pdl, s);
     }
     nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
     if (!virial) {                                           // NVE loop and force-only calls: the lean body
@@ -1022,6 +1032,7 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG>, dim3((unsigned)((n + LBT - 1) / LBT)),
                                   dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
                                   nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, nl->d_status));
+        nl->gather_pdl = 1;
         return MD_OK;
     }
     MD_TERSOFF_LAUNCH(4, 128, 168);
@@ -1034,15 +1045,16 @@ template <class T, class Rec>
 int launch_multi(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                  const double box[3], const int32_t* types, const md_tersoff_multi_params* mp, double* pe,
                  double* f, double* virial, cudaStream_t s) {
+    nl->gather_pdl = 0;
     const TersoffDev<T> p = make_dev<T>(&mp->elem[0]);       // used by the single-element register body only
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
     switch (mp->ntypes) {
-        case 1: return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, mp, nullptr, gtab, pe, f, virial, s);
-        case 2: return launch_sorted<T, Rec, 2>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
-        case 3: return launch_sorted<T, Rec, 3>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
-        default: return launch_sorted<T, Rec, 4>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, s);
+        case 1: return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, mp, nullptr, gtab, pe, f, virial, false, s);
+        case 2: return launch_sorted<T, Rec, 2>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, false, s);
+        case 3: return launch_sorted<T, Rec, 3>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, false, s);
+        default: return launch_sorted<T, Rec, 4>(nl, n, x, y, z, box, p, mp, types, gtab, pe, f, virial, false, s);
     }
 }
 
