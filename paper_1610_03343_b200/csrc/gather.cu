@@ -68,8 +68,11 @@ k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, 
 // this step and, unless it is the last step, the next step's kick + drift + wrap are applied before
 // anything is stored.  The arithmetic is operation for operation that of k_gather followed by k_kick and
 // k_kick_drift (integrate.cu), so the trajectory is bit-identical to the unfused composition.
+#ifndef MD_GVV_BT
+#define MD_GVV_BT 128
+#endif
 template <class T, class Rec, int MODE>
-__global__ void __launch_bounds__(256, 4)
+__global__ void __launch_bounds__(MD_GVV_BT, 1024 / MD_GVV_BT)
 k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int dense,   // Q, MASK, f: no __restrict__/.nc --
             double* f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,   // the pair kernel
             double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,           // before wrote them
@@ -138,7 +141,7 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
 #define MD_GATHER_VV(TT, RR, MODE)                                                                        \
-    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3(gb), dim3(256), 0, s, nl->gather_pdl != 0, n, nl->K, (const RR*)nl->Q,            \
+    MD_CUDA_TRY(md_launch_pdl(k_gather_vv<TT, RR, MODE>, dim3((unsigned)((n + MD_GVV_BT - 1) / MD_GVV_BT)), dim3(MD_GVV_BT), 0, s, nl->gather_pdl != 0, n, nl->K, (const RR*)nl->Q,            \
                               nl->MASK, nl->q_dense, f, vv->x, vv->y, vv->z, vv->vx, vv->vy, vv->vz, vv->hk, vv->dt,    \
                               box[0], box[1], box[2]))
         if (precision == MD_FP32) { if (vv->mode == 2) MD_GATHER_VV(float, float4, 2); else MD_GATHER_VV(float, float4, 1); }
