@@ -65,9 +65,12 @@ template <class T, class Rec>
 __device__ __noinline__ void
 tersoff_warp_atom(int64_t i, int64_t n, const double* x, const double* y, const double* z, double Lx, double Ly,
                   double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                  const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const fm::Tab& tb, Rec* __restrict__ Q,
+                  const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const double* tab_smem, Rec* __restrict__ Q,
                   unsigned long long* __restrict__ MASK, double* __restrict__ pe, double* __restrict__ f,
                   double* __restrict__ virial, int* __restrict__ status, WarpSlots& ws) {
+    fm::Tab tb;
+    tb.e = tab_smem;
+    tb.l = reinterpret_cast<const double2*>(tab_smem + fm::EXP_N);
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
@@ -180,21 +183,26 @@ tersoff_warp_atom(int64_t i, int64_t n, const double* x, const double* y, const 
 
 // The CTA's atoms that need the general path are queued (a shared-memory counter; the order in the queue does
 // not influence any result) and, after a barrier, taken one per warp.
-template <int BT>
-struct SlowQueue { WarpSlots ws[BT / 32]; int atom[BT]; int count; };
+template <class T, int BT>
+struct SlowQueue {
+    WarpSlots ws[BT / 32];
+    TersoffDev<T> p;          // the kernel's parameter block: handed to the non-inlined general path by address (as a
+    int atom[BT];             // by-value or by-reference argument every thread spilled its 112 bytes to local memory
+    int count;                // before the call, whether or not the queue held anything)
+};
 
 template <class T, class Rec, int BT>
 __device__ __forceinline__ void
-tersoff_drain_queue(SlowQueue<BT>& sq, int64_t n, const double* x, const double* y, const double* z, double Lx,
+tersoff_drain_queue(SlowQueue<T, BT>& sq, int64_t n, const double* x, const double* y, const double* z, double Lx,
                     double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-                    const uint8_t* __restrict__ REV, const TersoffDev<T>& p, const fm::Tab& tb, Rec* __restrict__ Q,
+                    const uint8_t* __restrict__ REV, const fm::Tab& tb, Rec* __restrict__ Q,
                     unsigned long long* __restrict__ MASK, double* __restrict__ pe, double* __restrict__ f,
                     double* __restrict__ virial, int* __restrict__ status) {
     __syncthreads();
     const int ns = sq.count, w = threadIdx.x >> 5;
     for (int k = w; k < ns; k += BT / 32)
-        tersoff_warp_atom<T, Rec>(sq.atom[k], n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, virial, status,
-                                  sq.ws[w]);
+        tersoff_warp_atom<T, Rec>(sq.atom[k], n, x, y, z, Lx, Ly, Lz, NN, NL, REV, sq.p, tb.e, Q, MASK, pe, f, virial,
+                                  status, sq.ws[w]);
 }
 
 // Register body: up to MR neighbour slots, every per-neighbour quantity in registers (all array indices are
@@ -374,8 +382,8 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
     // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
     // index and masked out below), and the table staging's barrier comes after the loads are in flight.
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
-    __shared__ SlowQueue<BT> s_slow;
-    if (threadIdx.x == 0) s_slow.count = 0;
+    __shared__ SlowQueue<T, BT> s_slow;
+    if (threadIdx.x == 0) { s_slow.count = 0; s_slow.p = p; }
     const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t i = i0 < n ? i0 : n - 1;
     const int nn = NN[i];
@@ -429,7 +437,7 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
     MASK[i] = (unsigned long long)mask;
     tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
     }
-    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, virial, status);
+    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, tb, Q, MASK, pe, f, virial, status);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -566,8 +574,8 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, int* __restrict__ status) {
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
-    __shared__ SlowQueue<BT> s_slow;
-    if (threadIdx.x == 0) s_slow.count = 0;
+    __shared__ SlowQueue<T, BT> s_slow;
+    if (threadIdx.x == 0) { s_slow.count = 0; s_slow.p = p; }
     const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t i = i0 < n ? i0 : n - 1;
     const int nn = NN[i];
@@ -624,7 +632,7 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
         tersoff_lean_body<T, Rec, MR>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f);
     }
     }
-    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, p, tb, Q, MASK, pe, f, nullptr, status);
+    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, tb, Q, MASK, pe, f, nullptr, status);
 }
 
 // Register path for a bin of atoms with at most MR in-range neighbours (pair_sort.cuh, Bins): thread t of CTA
