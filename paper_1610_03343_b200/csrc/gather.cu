@@ -11,56 +11,121 @@
 
 namespace {
 
-template <class T, class Rec>
-__global__ void __launch_bounds__(256)
-k_gather(int64_t n, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+// GEOM = false: forces only.  GEOM = true: virial and / or heat current too, which need r_ij of every in-range
+// neighbour (list entry -> coordinates, two dependent loads).  The first four record slots -- and, where the slot is
+// the list position (crystal kernels), their list entries -- are requested before MASK has arrived, the four
+// neighbours' coordinates together after it; only rows with more than four in-range neighbours enter the loop.
+// Sums run over the in-range slots in ascending order (as in k_gather_vv: bit-identical forces).
+template <class T, class Rec, bool GEOM>
+__global__ void __launch_bounds__(128)
+k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
          const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NL, const Rec* __restrict__ Q,
          const unsigned long long* __restrict__ MASK, int dense, double* __restrict__ f,
          double* __restrict__ virial, double* __restrict__ heat) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    T hx[4], hy[4], hz[4];
+    int hj[4];
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl) {
+        const int64_t row = (int64_t)(sl < K ? sl : 0) * n + i;
+        rm::load_rec(&Q[row], &hx[sl], &hy[sl], &hz[sl]);
+        hj[sl] = GEOM ? NL[row] : 0;                         // the list entry of slot sl if slot = list position
+    }
     unsigned long long mask = MASK[i];
-    const bool geom = virial != nullptr || heat != nullptr;
     double xi = 0, yi = 0, zi = 0;
     T vxi = T(0), vyi = T(0), vzi = T(0);
-    if (geom) { xi = x[i]; yi = y[i]; zi = z[i]; }
-    if (heat) { vxi = (T)vx[i]; vyi = (T)vy[i]; vzi = (T)vz[i]; }
+    // own halves the pair kernel left (read-modify-write at the end): requested now, not after the arithmetic
+    double of[3] = {0, 0, 0}, ow[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+    if (f) { of[0] = f[i]; of[1] = f[n + i]; of[2] = f[2 * n + i]; }
+    if (GEOM && virial) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) ow[q] = virial[(int64_t)q * n + i];
+    }
+    if (GEOM) { xi = x[i]; yi = y[i]; zi = z[i]; }
+    if (GEOM && heat) { vxi = (T)vx[i]; vyi = (T)vy[i]; vzi = (T)vz[i]; }
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
     T Jx = T(0), Jy = T(0), Jz = T(0);
-    int slot = 0;
-    while (mask) {
-        const int m = __ffsll((long long)mask) - 1;
-        mask &= mask - 1;
-        T px, py, pz;
-        rm::load_rec(&Q[(int64_t)(dense ? slot : m) * n + i], &px, &py, &pz);
-        ++slot;
-        Fx += px; Fy += py; Fz += pz;
-        if (geom) {
-            const int j = NL[(int64_t)m * n + i];
-            const T rx = (T)md_min_image(x[j] - xi, Lx, 0.5 * Lx);
-            const T ry = (T)md_min_image(y[j] - yi, Ly, 0.5 * Ly);
-            const T rz = (T)md_min_image(z[j] - zi, Lz, 0.5 * Lz);
-            if (virial) {
-                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
-                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
-                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+    auto geom_terms = [&](T px, T py, T pz, double qx, double qy, double qz) {
+        const T rx = (T)md_min_image(qx - xi, Lx, 0.5 * Lx);
+        const T ry = (T)md_min_image(qy - yi, Ly, 0.5 * Ly);
+        const T rz = (T)md_min_image(qz - zi, Lz, 0.5 * Lz);
+        if (virial) {
+            W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+            W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+            W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+        }
+        if (heat) {
+            const T dot = px * vxi + py * vyi + pz * vzi;
+            Jx += rx * dot; Jy += ry * dot; Jz += rz * dot;
+        }
+    };
+    // the first four slots
+    const int cnt = __popcll(mask);
+    bool use[4];
+    double qx[4], qy[4], qz[4];
+    {
+        unsigned long long run = mask;
+#pragma unroll
+        for (int sl = 0; sl < 4; ++sl) {
+            use[sl] = dense ? sl < cnt : (mask >> sl & 1ull) != 0;
+            if (GEOM) {
+                int j = hj[sl];
+                if (dense) {                                 // slot sl holds the sl-th in-range list entry
+                    const int m = run ? __ffsll((long long)run) - 1 : 0;
+                    run &= run - 1;
+                    j = NL[(int64_t)m * n + i];
+                }
+                j = use[sl] ? j : (int)i;
+                qx[sl] = x[j]; qy[sl] = y[j]; qz[sl] = z[j];
             }
-            if (heat) {
-                const T dot = px * vxi + py * vyi + pz * vzi;
-                Jx += rx * dot; Jy += ry * dot; Jz += rz * dot;
+        }
+    }
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl)
+        if (use[sl]) {
+            Fx += hx[sl]; Fy += hy[sl]; Fz += hz[sl];
+            if (GEOM) geom_terms(hx[sl], hy[sl], hz[sl], qx[sl], qy[sl], qz[sl]);
+        }
+    // rows with more in-range neighbours
+    if (dense) {
+        unsigned long long run = mask;
+        for (int sl = 0; sl < 4 && run; ++sl) run &= run - 1;
+        for (int sl = 4; sl < cnt; ++sl) {
+            const int m = __ffsll((long long)run) - 1;
+            run &= run - 1;
+            T px, py, pz;
+            rm::load_rec(&Q[(int64_t)sl * n + i], &px, &py, &pz);
+            Fx += px; Fy += py; Fz += pz;
+            if (GEOM) {
+                const int j = NL[(int64_t)m * n + i];
+                geom_terms(px, py, pz, x[j], y[j], z[j]);
+            }
+        }
+    } else {
+        mask &= ~15ull;
+        while (mask) {
+            const int m = __ffsll((long long)mask) - 1;
+            mask &= mask - 1;
+            T px, py, pz;
+            rm::load_rec(&Q[(int64_t)m * n + i], &px, &py, &pz);
+            Fx += px; Fy += py; Fz += pz;
+            if (GEOM) {
+                const int j = NL[(int64_t)m * n + i];
+                geom_terms(px, py, pz, x[j], y[j], z[j]);
             }
         }
     }
     if (f) {
-        f[i] -= (double)Fx; f[n + i] -= (double)Fy; f[2 * n + i] -= (double)Fz;
+        f[i] = of[0] - (double)Fx; f[n + i] = of[1] - (double)Fy; f[2 * n + i] = of[2] - (double)Fz;
     }
-    if (virial) {
+    if (GEOM && virial) {
 #pragma unroll
-        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] += (double)(T(0.5) * W[q]);
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = ow[q] + (double)(T(0.5) * W[q]);
     }
-    if (heat) { heat[i] = (double)Jx; heat[n + i] = (double)Jy; heat[2 * n + i] = (double)Jz; }
+    if (GEOM && heat) { heat[i] = (double)Jx; heat[n + i] = (double)Jy; heat[2 * n + i] = (double)Jz; }
 }
 
 // The same force sum with the velocity-Verlet half steps that follow it fused in (md_nve_run only, where
@@ -136,7 +201,6 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
                      const double* vx, const double* vy, const double* vz, const double box[3],
                      int precision, double* f, double* virial, double* heat, const VVFuse* vv, cudaStream_t s) {
     if (n == 0 || (!f && !virial && !heat)) return MD_OK;
-    const unsigned gb = (unsigned)((n + 255) / 256);
     ProfScope prof(nl, MD_KIND_GATHER, 1, s);
     if (vv) {
         if (!f || virial || heat) return MD_ERR_ARG;
@@ -150,12 +214,14 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
         MD_CUDA_TRY(cudaGetLastError());
         return MD_OK;
     }
-    if (precision == MD_FP32)
-        k_gather<float, float4><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
-                                                   (const float4*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat);
-    else
-        k_gather<double, PairRec64><<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,
-                                                       (const PairRec64*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat);
+    const unsigned gg = (unsigned)((n + 127) / 128);
+    const bool geom = virial != nullptr || heat != nullptr;
+#define MD_GATHER(TT, RR, GEOM)                                                                                   \
+    k_gather<TT, RR, GEOM><<<gg, 128, 0, s>>>(n, nl->K, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,      \
+                                              (const RR*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat)
+    if (precision == MD_FP32) { if (geom) MD_GATHER(float, float4, true); else MD_GATHER(float, float4, false); }
+    else { if (geom) MD_GATHER(double, PairRec64, true); else MD_GATHER(double, PairRec64, false); }
+#undef MD_GATHER
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;
 }
