@@ -109,6 +109,34 @@ def test_lean_register_kernel_next_to_general_path_atoms():
     assert_close_fp64("f", full["f"], ref["f"])
 
 
+def test_general_path_interstitial_ten_neighbours():
+    """An atom at the tetrahedral interstitial site has 10 neighbours inside the force range, 6 of them inside the
+    cut-off window; it and its neighbours (rows of 5..10 entries) take the warp-per-atom general path of both
+    register kernels while the other 4086 atoms take the register bodies; n = 4097 leaves a ragged last tile."""
+    s = mi.silicon_crystal(8, 0.05, 300.0, 33)
+    p = mi.TERSOFF_SI_C
+    for k in "xyz":
+        s[k] = np.append(s[k], 3.5 * mi.SI_LATTICE_A)
+    for k in ("vx", "vy", "vz"):
+        s[k] = np.append(s[k], 1e-3)
+    g = GpuSystem(s, 16)
+    g.build(mi.r_list("tersoff"))
+    max_row, long_rows = md.md_neighbors_row_stats(g.nl)
+    assert max_row >= 10 and long_rows * 256 <= g.n
+    NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], s["box"], mi.r_list("tersoff"), 16)
+    ref = oracle.evaluate("tersoff", p, s["x"], s["y"], s["z"], s["box"], NN, NL, v=(s["vx"], s["vy"], s["vz"]),
+                          precision="f80")
+    lean = g.force("tersoff", p, want=("pe", "f"))            # k_tersoff_lean + general path
+    full = g.force("tersoff", p)                              # k_tersoff_atom + general path, all outputs
+    for out in (lean, full):
+        assert_close_fp64("f", out["f"], ref["f"])
+        assert_close_energy(out["pe"], ref["pe"])
+    assert_close_fp64("virial", full["virial"], ref["virial"])
+    assert_close_fp64("heat", full["heat"], ref["heat"])
+    f32 = g.force("tersoff", p, precision=md.MD_FP32, want=("pe", "f"))
+    assert_close_fp32("f", f32["f"], ref["f"])
+
+
 def test_run_to_run_bitwise_reproducible():
     s = mi.silicon_crystal(6, 0.15, 1500.0, 77)
     a = GpuSystem(s, 16); a.build(3.5); oa = a.force("tersoff", mi.TERSOFF_SI_C)
