@@ -19,7 +19,7 @@
 
 namespace ps {
 
-// d2 of a listed pair, the same roundings wherever MASK is decided (k_tersoff_atom, the generic path, the
+// d2 of a listed pair, the same roundings wherever MASK is decided (k_tersoff_lean, the warp-per-atom general path, the
 // screen below): dx*dx rounded, then two fused multiply-adds.  x_j - x_i and the minimum-image shift are exact
 // negations of each other for (i,j) and (j,i), so both ends compute the same bits.
 __device__ __forceinline__ double in_range_d2(double dx, double dy, double dz) {

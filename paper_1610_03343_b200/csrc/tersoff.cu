@@ -368,78 +368,6 @@ tersoff_reg_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], un
 }
 
 
-// Thread-per-atom kernel for crystal rows (at most MR listed entries): slot m is list position m.
-template <class T, class Rec, int MR, int BT, int MAXREG>
-__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
-k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__: see below
-               double Lx, double Ly, double Lz,
-               const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
-               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial,
-               int* __restrict__ status) {
-    // Loads first, in two dependent levels only: {NN, NL, REV, math tables} -> {x[j]}.  The list slots are
-    // read without waiting for NN (a slot past the row's end holds anything: it is clamped to a valid
-    // index and masked out below), and the table staging's barrier comes after the loads are in flight.
-    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
-    __shared__ SlowQueue<T, BT> s_slow;
-    if (threadIdx.x == 0) { s_slow.count = 0; s_slow.p = p; }
-    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const int64_t i = i0 < n ? i0 : n - 1;
-    const int nn = NN[i];
-    int jd[MR], rv[MR];
-#pragma unroll
-    for (int m = 0; m < MR; ++m) {
-        const int mk = m < K ? m : 0;
-        const int jr = NL[(int64_t)mk * n + i];
-        jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
-        rv[m] = (int)REV[(int64_t)mk * n + i];
-    }
-    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
-    // Inside md_nve_run this kernel is launched as a programmatic dependent of the fused gather kernel that
-    // wrote x, y, z (common.cuh, md_launch_pdl): the list loads above overlap with that kernel's tail; the
-    // coordinates are read only from here on, through plain (coherent, non-.nc) loads.
-    md_grid_wait();
-    md_grid_release();
-    const double xi = x[i], yi = y[i], zi = z[i];
-    double dx[MR], dy[MR], dz[MR];
-#pragma unroll
-    for (int m = 0; m < MR; ++m) { dx[m] = x[jd[m]]; dy[m] = y[jd[m]]; dz[m] = z[jd[m]]; }   // all loads in flight
-    __syncthreads();
-    if (i0 < n && nn > MR) s_slow.atom[atomicAdd(&s_slow.count, 1)] = (int)i;   // rows longer than MR: the general path
-    if (i0 < n && nn <= MR) {
-    const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
-    T ex[MR], ey[MR], ez[MR];
-    unsigned mask = 0u;
-    {
-        double qx[MR], qy[MR], qz[MR];
-        T d2[MR];
-        bool far = false;
-#pragma unroll
-        for (int m = 0; m < MR; ++m) {
-            qx[m] = dx[m] - xi; qy[m] = dy[m] - yi; qz[m] = dz[m] - zi;
-            d2[m] = ps::in_range_d2((T)qx[m], (T)qy[m], (T)qz[m]);       // the one in-range decision (pair_sort.cuh)
-            far = far || mi.far(d2[m]);
-        }
-        if (__any_sync(__activemask(), far)) {               // warp-uniform: interior warps never shift
-#pragma unroll
-            for (int m = 0; m < MR; ++m) {
-                mi.wrap(qx[m], qy[m], qz[m]);
-                d2[m] = ps::in_range_d2((T)qx[m], (T)qy[m], (T)qz[m]);
-            }
-        }
-#pragma unroll
-        for (int m = 0; m < MR; ++m) {
-            ex[m] = (T)qx[m]; ey[m] = (T)qy[m]; ez[m] = (T)qz[m];
-            mask |= (m < nn && d2[m] < p.S2) ? 1u << m : 0u;
-        }
-    }
-    MASK[i] = (unsigned long long)mask;
-    tersoff_reg_body<T, Rec, MR>(i, n, ex, ey, ez, mask, jd, rv, p, tb, Q, pe, f, virial);
-    }
-    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, tb, Q, MASK, pe, f, virial, status);
-}
-
 // ---------------------------------------------------------------------------------------------------
 // Lean register body: the crystal case of the NVE loop and of force-only calls (no virial asked for, no pair
 // inside the cut-off window R < r < S).  Then f_C is 1 or 0 and f_C' = 0 for every slot, so f_C, f_C', r and
@@ -447,11 +375,11 @@ k_tersoff_atom(int64_t n, int K, const double* x, const double* y, const double*
 // index and reverse slot fold into ONE 32-bit record index per slot, and the body fits 128 registers: 4 CTAs
 // of 128 threads per SM instead of 3 (the kernel is bound by latency, not by the FP64 pipe: ncu r02a).  An
 // atom with a pair inside the window is handed to the general per-thread path before any arithmetic.
-template <class T, class Rec, int MR>
+template <class T, class Rec, int MR, bool WITH_W>
 __device__ __forceinline__ void
 tersoff_lean_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], const T (&d2in)[MR], unsigned mask,
                   const unsigned (&qi)[MR], const TersoffDev<T>& p, const fm::Tab& tb,
-                  Rec* __restrict__ Q, double* __restrict__ pe, double* __restrict__ f) {
+                  Rec* __restrict__ Q, double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial) {
     constexpr int NP = MR * (MR - 1) / 2;
     T rinv[MR], fR[MR], fA[MR], zeta[MR];
     {
@@ -563,16 +491,30 @@ tersoff_lean_body(int64_t i, int64_t n, T (&ex)[MR], T (&ey)[MR], T (&ez)[MR], c
         }
     if (pe) pe[i] = (double)U;
     if (f) { f[i] = (double)Fx; f[n + i] = (double)Fy; f[2 * n + i] = (double)Fz; }
+    if (WITH_W) {                                            // own half -1/2 sum_a r_a (x) P_a; r_a = e_a d2_a / r_a
+        T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+#pragma unroll
+        for (int a = 0; a < MR; ++a)
+            if (mask >> a & 1u) {
+                const T rr = d2in[a] * rinv[a];
+                const T rx = ex[a] * rr, ry = ey[a] * rr, rz = ez[a] * rr;
+                W[0] += rx * Px[a]; W[1] += rx * Py[a]; W[2] += rx * Pz[a];
+                W[3] += ry * Px[a]; W[4] += ry * Py[a]; W[5] += ry * Pz[a];
+                W[6] += rz * Px[a]; W[7] += rz * Py[a]; W[8] += rz * Pz[a];
+            }
+#pragma unroll
+        for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
+    }
 }
 
-template <class T, class Rec, int MR, int BT, int MAXREG>
+template <class T, class Rec, int MR, int BT, int MAXREG, bool WITH_W>
 __global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
-k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__: as k_tersoff_atom
+k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__ (see the wait below)
                double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
                const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
                Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
-               double* __restrict__ pe, double* __restrict__ f, int* __restrict__ status) {
+               double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial, int* __restrict__ status) {
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
     __shared__ SlowQueue<T, BT> s_slow;
     if (threadIdx.x == 0) { s_slow.count = 0; s_slow.p = p; }
@@ -589,7 +531,10 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
         qi[m] = (unsigned)REV[(int64_t)mk * n + i] * (unsigned)n + (unsigned)jd[m];   // n * K <= 2e9 (md_neighbors_create)
     }
     const fm::Tab tb = fm::stage_tables(s_tab, gtab);
-    md_grid_wait();                                          // programmatic dependent of the fused gather (see k_tersoff_atom)
+    // Inside md_nve_run this kernel is launched as a programmatic dependent of the fused gather kernel that
+    // wrote x, y, z (common.cuh, md_launch_pdl): the list loads above overlap with that kernel's tail; the
+    // coordinates are read only from here on, through plain (coherent, non-.nc) loads.
+    md_grid_wait();
     md_grid_release();
     const double xi = x[i], yi = y[i], zi = z[i];
     double dx[MR], dy[MR], dz[MR];
@@ -629,10 +574,11 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
         s_slow.atom[atomicAdd(&s_slow.count, 1)] = (int)i;
     } else {
         MASK[i] = (unsigned long long)mask;
-        tersoff_lean_body<T, Rec, MR>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f);
+        tersoff_lean_body<T, Rec, MR, WITH_W>(i, n, ex, ey, ez, d2, mask, qi, p, tb, Q, pe, f, virial);
     }
     }
-    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, tb, Q, MASK, pe, f, nullptr, status);
+    tersoff_drain_queue<T, Rec, BT>(s_slow, n, x, y, z, Lx, Ly, Lz, NN, NL, REV, tb, Q, MASK, pe, f, WITH_W ? virial : nullptr,
+                                    status);
 }
 
 // Register path for a bin of atoms with at most MR in-range neighbours (pair_sort.cuh, Bins): thread t of CTA
@@ -1018,10 +964,6 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
     ProfScope prof(nl, MD_KIND_PAIR, 1, s);
     const double* gtab = md_math_tables();
     if (!gtab) return MD_ERR_ALLOC;
-#define MD_TERSOFF_LAUNCH(MRV, BT, MAXREG)                                                                 \
-    MD_CUDA_TRY(md_launch_pdl(k_tersoff_atom<T, Rec, MRV, BT, MAXREG>, dim3((unsigned)((n + BT - 1) / BT)), dim3(BT), 0, s, pdl, \
-                              n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, gtab,   \
-                              (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status))
     // Kernel selection by the row lengths of the list (known on the host once per build): the register
     // kernel handles rows of up to 4 entries (the crystal) in its fast path and longer ones through a slow
     // per-thread fallback, so it is used while fewer than 1 row in 256 is longer; otherwise the
@@ -1035,18 +977,19 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         return launch_sorted<T, Rec, 1>(nl, n, x, y, z, box, p, &one, nullptr, gtab, pe, f, virial, pdl, s);
     }
     nl->q_dense = 0;                                         // slot = reverse position (rows are at most 4 long)
-    if (!virial) {                                           // NVE loop and force-only calls: the lean body
+    {   // the lean body; with the virial own half as a second instantiation (both fit 128 registers)
         constexpr int LBT = MD_TERSOFF_LEAN_BT;
-        MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG>, dim3((unsigned)((n + LBT - 1) / LBT)),
-                                  dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
-                                  nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, nl->d_status));
+        if (virial)
+            MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG, true>, dim3((unsigned)((n + LBT - 1) / LBT)),
+                                      dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
+                                      nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
+        else
+            MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG, false>, dim3((unsigned)((n + LBT - 1) / LBT)),
+                                      dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
+                                      nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
         nl->gather_pdl = 1;
         return MD_OK;
     }
-    MD_TERSOFF_LAUNCH(4, 128, 168);
-#undef MD_TERSOFF_LAUNCH
-    MD_CUDA_TRY(cudaGetLastError());
-    return MD_OK;
 }
 
 template <class T, class Rec>

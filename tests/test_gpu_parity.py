@@ -105,7 +105,7 @@ def test_lean_register_kernel_next_to_general_path_atoms():
         out = g.force("tersoff", p, want=("pe", "f"))
         assert_close_fp64("f", out["f"], ref["f"])
         assert_close_energy(out["pe"], ref["pe"])
-    full = g.force("tersoff", p)                              # the 168-register kernel (virial asked for)
+    full = g.force("tersoff", p)                              # the instantiation with the virial own half
     assert_close_fp64("f", full["f"], ref["f"])
 
 
@@ -127,7 +127,7 @@ def test_general_path_interstitial_ten_neighbours():
     ref = oracle.evaluate("tersoff", p, s["x"], s["y"], s["z"], s["box"], NN, NL, v=(s["vx"], s["vy"], s["vz"]),
                           precision="f80")
     lean = g.force("tersoff", p, want=("pe", "f"))            # k_tersoff_lean + general path
-    full = g.force("tersoff", p)                              # k_tersoff_atom + general path, all outputs
+    full = g.force("tersoff", p)                              # k_tersoff_lean with the virial own half + general path
     for out in (lean, full):
         assert_close_fp64("f", out["f"], ref["f"])
         assert_close_energy(out["pe"], ref["pe"])
