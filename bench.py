@@ -453,6 +453,41 @@ def measure_literal_ab(gpu, md, cfg_index, calls, warmup):
     return out
 
 
+def measure_ensembles(gpu, md, cfg_index, steps, warmup):
+    """md_npt_run (Berendsen NPT, the paper's benchmark ensemble: velocity-Verlet + per-atom
+    virial + two scalars read back per step) and md_nve_heat_run (Green-Kubo sampling every 10th step) on the
+    headline workload, in atom-steps/s, one call of `steps` steps each, CUDA events around the call."""
+    torch = gpu.torch
+    c = mi.make_config(cfg_index)
+    pot, n, K = c["potential"], c["n"], c["max_neighbors"]
+    out = {"workload": c["name"], "atoms": n, "steps": steps}
+    ber = dict(T0=300.0, tau_T=100.0, P0=0.0, tau_P=1000.0, beta=1.0 / 0.6104)
+    for name in ("npt_berendsen", "nve_green_kubo_every_10"):
+        d = {k: torch.from_numpy(c[k].copy()).to(gpu.dev) for k in ("x", "y", "z", "vx", "vy", "vz")}
+        f = torch.zeros((3, n), dtype=torch.float64, device=gpu.dev)
+        nl = md.md_neighbors_create(n, K)
+        box = list(c["box"])
+
+        def run(first, nsteps, f_valid):
+            if name == "npt_berendsen":
+                md.md_npt_run(nl, pot, c["params"], n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], f, f_valid, box,
+                              c["mass"], c["dt"], nsteps, c["rebuild_every"], c["r_list"], ber, first_step=first)
+            else:
+                md.md_nve_heat_run(nl, pot, c["params"], n, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"], f, f_valid,
+                                   box, c["mass"], c["dt"], nsteps, c["rebuild_every"], c["r_list"], 10, first_step=first)
+        run(0, warmup, False)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        gpu.barrier()
+        gpu.flush_l2()
+        e0.record(); run(warmup, steps, True); e1.record()
+        torch.cuda.synchronize()
+        ms, = gpu_max([e0.elapsed_time(e1)], gpu)
+        md.md_neighbors_status(nl)
+        md.md_neighbors_destroy(nl)
+        out[name] = {"value": gpu.world * n * steps / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms / steps}
+    return out
+
+
 def summary(r):
     """The per-config entry of the line's `configs` object."""
     c = r["c"]
@@ -499,6 +534,7 @@ def main_ours(args):
         extra["cfg1_tersoff_512_eval"] = measure_eval(gpu, md, 0, 200, args.warmup, fp64_peak, peaks)
         extra["cfg2_size_full_output_eval"] = measure_eval(gpu, md, 1, 20, args.warmup, fp64_peak, peaks)
         extra["multi_element_sic_512k_eval"] = measure_multi_eval(gpu, md, 20, args.warmup, peaks)
+        extra["ensembles_cfg2"] = measure_ensembles(gpu, md, 1, 100, 20)
         extra["literal_vs_stored_P_cfg2"] = measure_literal_ab(gpu, md, 1, 20, args.warmup)
         extra["literal_vs_stored_P_cfg4"] = measure_literal_ab(gpu, md, 3, 5, args.warmup)
     if gpu.rank != 0:
