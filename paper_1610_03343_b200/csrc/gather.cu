@@ -165,10 +165,13 @@ k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int 
 #pragma unroll
         for (int sl = 0; sl < 4; ++sl)
             if (sl < cnt) { Fx += hx[sl]; Fy += hy[sl]; Fz += hz[sl]; }
-        for (int sl = 4; sl < cnt; ++sl) {
-            T qx, qy, qz;
-            rm::load_rec(&Q[(int64_t)sl * n + i], &qx, &qy, &qz);
-            Fx += qx; Fy += qy; Fz += qz;
+        for (int s0 = 4; s0 < cnt; s0 += 4) {                // the rest four at a time: loads first, sums in slot order
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                rm::load_rec(&Q[(int64_t)(s0 + u < cnt ? s0 + u : s0) * n + i], &hx[u], &hy[u], &hz[u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (s0 + u < cnt) { Fx += hx[u]; Fy += hy[u]; Fz += hz[u]; }
         }
     } else {                                                 // slot = list position
 #pragma unroll
