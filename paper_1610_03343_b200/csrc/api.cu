@@ -442,6 +442,7 @@ int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int pre
         if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
         if ((step - first_step + 1) % sample_every != 0) continue;
         // Eq. (30) with the velocities of this state: the pair records are still valid, one more gather
+        nl->gather_pdl = 0;                                   // the kernel before (the kick) wrote the velocities it reads
         if ((rc = md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, nullptr, nullptr, J, nullptr, s)) != MD_OK)
             return rc;
         // U_i of this state for the convective part (a second pair pass: the fused NVE path never stores it)

@@ -20,22 +20,28 @@ template <class T, class Rec, bool GEOM>
 __global__ void __launch_bounds__(128)
 k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
          const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
-         double Lx, double Ly, double Lz, const int32_t* __restrict__ NL, const Rec* __restrict__ Q,
-         const unsigned long long* __restrict__ MASK, int dense, double* __restrict__ f,
-         double* __restrict__ virial, double* __restrict__ heat) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    T hx[4], hy[4], hz[4];
+         double Lx, double Ly, double Lz, const int32_t* __restrict__ NL, const Rec* Q,
+         const unsigned long long* MASK, int dense, double* f, double* virial,    // Q, MASK, f, virial: plain loads --
+         double* __restrict__ heat) {                                              // the pair kernel before wrote them
+    const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = i0 < n ? i0 : n - 1;
+    // Launched as a programmatic dependent of the pair kernel (common.cuh, md_launch_pdl): what that kernel does
+    // not write -- the list entries of the first four slots, the atom's position and velocity -- is requested
+    // while it drains.
     int hj[4];
 #pragma unroll
-    for (int sl = 0; sl < 4; ++sl) {
-        const int64_t row = (int64_t)(sl < K ? sl : 0) * n + i;
-        rm::load_rec(&Q[row], &hx[sl], &hy[sl], &hz[sl]);
-        hj[sl] = GEOM ? NL[row] : 0;                         // the list entry of slot sl if slot = list position
-    }
-    unsigned long long mask = MASK[i];
+    for (int sl = 0; sl < 4; ++sl) hj[sl] = GEOM ? NL[(int64_t)(sl < K ? sl : 0) * n + i] : 0;   // slot = list position
     double xi = 0, yi = 0, zi = 0;
     T vxi = T(0), vyi = T(0), vzi = T(0);
+    if (GEOM) { xi = x[i]; yi = y[i]; zi = z[i]; }
+    if (GEOM && heat) { vxi = (T)vx[i]; vyi = (T)vy[i]; vzi = (T)vz[i]; }
+    md_grid_wait();
+    md_grid_release();
+    if (i0 >= n) return;
+    T hx[4], hy[4], hz[4];
+#pragma unroll
+    for (int sl = 0; sl < 4; ++sl) rm::load_rec(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
+    unsigned long long mask = MASK[i];
     // own halves the pair kernel left (read-modify-write at the end): requested now, not after the arithmetic
     double of[3] = {0, 0, 0}, ow[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     if (f) { of[0] = f[i]; of[1] = f[n + i]; of[2] = f[2 * n + i]; }
@@ -43,8 +49,6 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
 #pragma unroll
         for (int q = 0; q < 9; ++q) ow[q] = virial[(int64_t)q * n + i];
     }
-    if (GEOM) { xi = x[i]; yi = y[i]; zi = z[i]; }
-    if (GEOM && heat) { vxi = (T)vx[i]; vyi = (T)vy[i]; vzi = (T)vz[i]; }
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
     T Jx = T(0), Jy = T(0), Jz = T(0);
@@ -220,8 +224,9 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
     const unsigned gg = (unsigned)((n + 127) / 128);
     const bool geom = virial != nullptr || heat != nullptr;
 #define MD_GATHER(TT, RR, GEOM)                                                                                   \
-    k_gather<TT, RR, GEOM><<<gg, 128, 0, s>>>(n, nl->K, x, y, z, vx, vy, vz, box[0], box[1], box[2], nl->NL,      \
-                                              (const RR*)nl->Q, nl->MASK, nl->q_dense, f, virial, heat)
+    MD_CUDA_TRY(md_launch_pdl(k_gather<TT, RR, GEOM>, dim3(gg), dim3(128), 0, s, nl->gather_pdl != 0, n, nl->K, x, y, z, vx, vy, vz,       \
+                              box[0], box[1], box[2], (const int32_t*)nl->NL, (const RR*)nl->Q,                   \
+                              (const unsigned long long*)nl->MASK, nl->q_dense, f, virial, heat))
     if (precision == MD_FP32) { if (geom) MD_GATHER(float, float4, true); else MD_GATHER(float, float4, false); }
     else { if (geom) MD_GATHER(double, PairRec64, true); else MD_GATHER(double, PairRec64, false); }
 #undef MD_GATHER
