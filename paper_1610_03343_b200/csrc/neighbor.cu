@@ -113,7 +113,7 @@ __global__ void k_scan_tiles(int32_t* __restrict__ tile_sums, int ntiles) {
     }
 }
 
-__global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t* __restrict__ tile_sums,
+__global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t* tile_sums,   // plain loads: note below
                            int32_t grand_total) {
     md_grid_wait();                                          // chained build kernels: see md_launch_build
     md_grid_release();
@@ -127,7 +127,7 @@ __global__ void k_scan_add(int32_t* __restrict__ data, int64_t n, const int32_t*
 
 __global__ void k_scatter(int64_t n, const double* __restrict__ x, const double* __restrict__ y,
                           const double* __restrict__ z, const int32_t* __restrict__ cell_of,
-                          const int32_t* __restrict__ rank, const int32_t* __restrict__ cell_start,
+                          const int32_t* __restrict__ rank, const int32_t* cell_start,
                           double4* __restrict__ sorted, float4* __restrict__ sortedf) {
     md_grid_wait();                                          // chained build kernels: see md_launch_build
     md_grid_release();
@@ -148,7 +148,7 @@ constexpr int SEARCH_BT = 128;
 #define SEARCH_MIN_CTAS 8
 #endif
 __global__ void __launch_bounds__(SEARCH_BT, SEARCH_MIN_CTAS)
-k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __restrict__ sortedf,
+k_search(int64_t n, Grid g, const double4* sorted, const float4* sortedf,
          const int32_t* __restrict__ cell_start, int K, float rc2_lo, float rc2_hi, int32_t* __restrict__ NN,
          int32_t* __restrict__ NL, int* __restrict__ status) {
     md_grid_wait();
@@ -277,7 +277,7 @@ k_search(int64_t n, Grid g, const double4* __restrict__ sorted, const float4* __
 // MD_DEV_NO_REVERSE.  Lists built by k_search are symmetric by construction (the predicate is) and skip that.
 template <bool CHECK>
 __global__ void __launch_bounds__(128)
-k_reverse(int64_t n, int K, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
+k_reverse(int64_t n, int K, const int32_t* NN, const int32_t* NL,
           uint8_t* __restrict__ REV, int* __restrict__ status) {
     md_grid_wait();
     md_grid_release();
@@ -399,6 +399,9 @@ int md_launch_build(md_neighbors* nl, int64_t n, const double* x, const double* 
     {
     ProfScope prof(nl, MD_KIND_BUILD, 6, s);
     MD_CUDA_TRY(cudaMemsetAsync(nl->cell_count, 0, sizeof(int32_t) * (ncell + 1), s));
+    // (What a kernel reads from the kernel directly before it is passed without __restrict__, so that it is read
+    // by plain coherent loads after the wait, never through the non-coherent path: tile_sums in k_scan_add,
+    // cell_start in k_scatter, sorted / sortedf in k_search, NN / NL in k_reverse.)
     // The seven kernels of a build each need everything the one before wrote, so each starts with
     // griddepcontrol.wait and is launched as a programmatic dependent: only the launch latency and ramp of the
     // next kernel overlap with the drain of the previous one (k_bin follows a memset and is launched normally).
