@@ -182,8 +182,10 @@ int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int pre
 
 /* End-to-end variant with HOST buffers (pinned or pageable): copies x,y,z,vx,vy,vz to the device,
  * runs md_nve_run from scratch (f_valid = 0), copies x,y,z,vx,vy,vz, f[3][n] and pe[n] back and
- * synchronises.  Device buffers are owned by the handle.  Returns the latched device status (as
- * md_neighbors_status would) since it has synchronised anyway. */
+ * synchronises.  Device buffers are owned by the handle.  The velocities are uploaded on a second, handle-owned
+ * stream and joined before the first kick, so the list build and the first force evaluation (positions only)
+ * overlap with that half of the transfer.  Returns the latched device status (as md_neighbors_status would)
+ * since it has synchronised anyway. */
 int md_nve_run_host(md_neighbors* nl, int potential, const void* params, int precision, int64_t n,
                     double* x, double* y, double* z, double* vx, double* vy, double* vz,
                     double* f, double* pe, const double box[3], double mass_amu, double dt_fs,
