@@ -169,7 +169,8 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
                const md_berendsen_params* b, double* T_trace, double* P_trace, void* stream);
 
 /* Green-Kubo workload (the application of the paper's Ref. [27]): NVE steps as
- * md_nve_run (unfused), and after every `sample_every`-th step the total heat current of that state:
+ * md_nve_run (the steps between two samples run as one fused segment), and after every `sample_every`-th step the
+ * total heat current of that state:
  *   J_pot = sum_i J_i (Eq. 30)      J_kin = sum_i (m v_i^2 / 2 + U_i) v_i   (convective part)
  * in eV A/fs.  J_pot, J_kin: HOST [nsteps / sample_every][3] (either may be NULL).  Reads six scalars back per
  * sample, so it synchronises `stream`.  The autocorrelation and its integral are the caller's

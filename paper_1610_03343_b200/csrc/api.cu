@@ -1,5 +1,6 @@
 // api.cu -- the C ABI declared in include/md.h: argument checks, handle life cycle, and the host-side
 // composition of the kernels.  No arithmetic of the method lives here.
+#include <algorithm>
 #include <cmath>
 #include <mutex>
 #include <new>
@@ -426,28 +427,20 @@ int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int pre
     }
     double* J = nl->npt_w;
     double* pe = nl->npt_w + 3 * n;
-    int rc, ns = 0;
-    if (!f_valid) {
-        if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
-        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
-                                 nullptr, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
-    }
-    for (int step = first_step; step < first_step + nsteps; ++step) {
-        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
-        if (step % rebuild_every == 0)
-            if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
-        if (nl->n != n) return MD_ERR_NO_LIST;
-        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
-                                 nullptr, f, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
-        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
-        if ((step - first_step + 1) % sample_every != 0) continue;
-        // Eq. (30) with the velocities of this state: the pair records are still valid, one more gather
-        nl->gather_pdl = 0;                                   // the kernel before (the kick) wrote the velocities it reads
+    // The steps between two samples run as one fused md_nve_run segment (pair kernel + fused gather per step,
+    // chained as programmatic dependents); its last step leaves the forces, U_i and -- still valid -- the pair
+    // records of the sampled state, so a sample costs one more gather (Eq. 30 with that state's velocities) and
+    // the reduction.  The trajectory is bit-identical to the unfused composition (tests/test_gpu_parity.py).
+    int rc, ns = 0, done = 0, fv = f_valid;
+    while (done < nsteps) {
+        const int seg = std::min(sample_every - done % sample_every, nsteps - done);
+        if ((rc = nve_run_impl(nl, potential, params, precision, n, x, y, z, vx, vy, vz, f, fv, pe, box, mass_amu, dt_fs,
+                               first_step + done, seg, rebuild_every, r_list, stream, nullptr)) != MD_OK) return rc;
+        done += seg; fv = 1;
+        if (done % sample_every != 0) break;                  // a trailing partial segment: no sample
+        nl->gather_pdl = 0;                                   // the kernel before (the last kick) wrote the velocities it reads
         if ((rc = md_launch_gather(nl, n, x, y, z, vx, vy, vz, box, precision, nullptr, nullptr, J, nullptr, s)) != MD_OK)
             return rc;
-        // U_i of this state for the convective part (a second pair pass: the fused NVE path never stores it)
-        if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
-                                 pe, nullptr, nullptr, nullptr, nullptr, s)) != MD_OK) return rc;
         double out[6];
         if ((rc = md_launch_heat_sums(nl, n, vx, vy, vz, pe, J, mass_amu, out, s)) != MD_OK) return rc;
         for (int a = 0; a < 3; ++a) {
