@@ -375,26 +375,30 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
     }
+    // Per step: kick+drift (with the scaling the step before decided applied first, in the same pass), [rebuild],
+    // force with W, then ONE pass that does the second half-kick and the two sums, two scalars to the host,
+    // lambda and mu for the next kick+drift.  Operation for operation the unfused sequence (kick; sums; scale).
+    const double hk = 0.5 * dt_fs * MD_KAPPA / mass_amu;
+    double lam_p = 1.0, mu_p = 1.0;
     for (int step = first_step; step < first_step + nsteps; ++step) {
-        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
+        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s, lam_p, mu_p)) != MD_OK) return rc;
         if (step % rebuild_every == 0)
             if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if (nl->n != n) return MD_ERR_NO_LIST;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
-        if ((rc = md_launch_vv(nl, 1, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s)) != MD_OK) return rc;
         double sums[2];
-        if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, sums, s)) != MD_OK) return rc;
+        if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, f, hk, sums, s)) != MD_OK) return rc;
         const double ke2 = sums[0] * mass_amu / MD_KAPPA;                 // 2 KE
         const double V = box[0] * box[1] * box[2];
         const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + sums[1]) / (3.0 * V);
         if (T_trace) T_trace[step - first_step] = T;
         if (P_trace) P_trace[step - first_step] = P;
-        const double lam = T > 0 ? sqrt(1.0 + dt_fs / b->tau_T * (b->T0 / T - 1.0)) : 1.0;
-        const double mu = cbrt(1.0 - b->beta * dt_fs / b->tau_P * (b->P0 - P));
-        if ((rc = md_launch_npt_scale(nl, n, x, y, z, vx, vy, vz, lam, mu, s)) != MD_OK) return rc;
-        for (int a = 0; a < 3; ++a) box[a] *= mu;
+        lam_p = T > 0 ? sqrt(1.0 + dt_fs / b->tau_T * (b->T0 / T - 1.0)) : 1.0;
+        mu_p = cbrt(1.0 - b->beta * dt_fs / b->tau_P * (b->P0 - P));
+        for (int a = 0; a < 3; ++a) box[a] *= mu_p;
     }
+    if (nsteps > 0 && (rc = md_launch_npt_scale(nl, n, x, y, z, vx, vy, vz, lam_p, mu_p, s)) != MD_OK) return rc;
     return MD_OK;
 }
 

@@ -170,11 +170,12 @@ int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double*
                      const double* vx, const double* vy, const double* vz, const double box[3],
                      int precision, double* f, double* virial, double* heat, const VVFuse* vv, cudaStream_t s);
 int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
-                 const double* f, double mass, double dt, const double box[3], cudaStream_t s);
+                 const double* f, double mass, double dt, const double box[3], cudaStream_t s,
+                 double lam = 1.0, double mu = 1.0);   // phase 0 only: v *= lam, x *= mu first (Berendsen scaling of md_npt_run)
 const double* md_math_tables();   // device tables of fastmath.cuh for the current device (nullptr on failure)
 int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);
-int md_launch_npt_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
-                       const double* W, double out[2], cudaStream_t s);
+int md_launch_npt_sums(md_neighbors* nl, int64_t n, double* vx, double* vy, double* vz,
+                       const double* W, const double* f, double hk, double out[2], cudaStream_t s);
 int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
                         double* vz, double lam, double mu, cudaStream_t s);
 int md_launch_heat_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,

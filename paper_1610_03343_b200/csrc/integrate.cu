@@ -5,14 +5,17 @@ namespace {
 
 __global__ void k_kick_drift(int64_t n, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
                              double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
-                             const double* __restrict__ f, double hk, double dt, double Lx, double Ly, double Lz) {
+                             const double* __restrict__ f, double hk, double dt, double Lx, double Ly, double Lz,
+                             double lam, double mu) {
+    // lam, mu: the weak-coupling scaling of the step before (md_npt_run), applied first; 1.0 (exact) otherwise
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const double ux = __fma_rn(hk, f[i], vx[i]) , uy = __fma_rn(hk, f[n + i], vy[i]), uz = __fma_rn(hk, f[2 * n + i], vz[i]);
+    const double ux = __fma_rn(hk, f[i], __dmul_rn(vx[i], lam)), uy = __fma_rn(hk, f[n + i], __dmul_rn(vy[i], lam)),
+                 uz = __fma_rn(hk, f[2 * n + i], __dmul_rn(vz[i], lam));
     vx[i] = ux; vy[i] = uy; vz[i] = uz;
-    x[i] = md_wrap(__fma_rn(dt, ux, x[i]), Lx);
-    y[i] = md_wrap(__fma_rn(dt, uy, y[i]), Ly);
-    z[i] = md_wrap(__fma_rn(dt, uz, z[i]), Lz);
+    x[i] = md_wrap(__fma_rn(dt, ux, __dmul_rn(x[i], mu)), Lx);
+    y[i] = md_wrap(__fma_rn(dt, uy, __dmul_rn(y[i], mu)), Ly);
+    z[i] = md_wrap(__fma_rn(dt, uz, __dmul_rn(z[i], mu)), Lz);
 }
 
 __global__ void k_kick(int64_t n, double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
@@ -26,12 +29,12 @@ __global__ void k_kick(int64_t n, double* __restrict__ vx, double* __restrict__ 
 }  // namespace
 
 int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
-                 const double* f, double mass, double dt, const double box[3], cudaStream_t s) {
+                 const double* f, double mass, double dt, const double box[3], cudaStream_t s, double lam, double mu) {
     if (n == 0) return MD_OK;
     const double hk = 0.5 * dt * MD_KAPPA / mass;
     const unsigned gb = (unsigned)((n + 255) / 256);
     ProfScope prof(nl, MD_KIND_INTEGRATE, 1, s);
-    if (phase == 0) k_kick_drift<<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, f, hk, dt, box[0], box[1], box[2]);
+    if (phase == 0) k_kick_drift<<<gb, 256, 0, s>>>(n, x, y, z, vx, vy, vz, f, hk, dt, box[0], box[1], box[2], lam, mu);
     else k_kick<<<gb, 256, 0, s>>>(n, vx, vy, vz, f, hk);
     MD_CUDA_TRY(cudaGetLastError());
     return MD_OK;

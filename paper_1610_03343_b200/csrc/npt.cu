@@ -9,12 +9,17 @@ namespace {
 constexpr int RED_BLOCKS = 296, RED_BT = 256;
 
 __global__ void __launch_bounds__(RED_BT)
-k_npt_partial(int64_t n, const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
-              const double* __restrict__ W, double* __restrict__ part) {
+k_npt_partial(int64_t n, double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
+              const double* __restrict__ W, const double* __restrict__ f, double hk, double* __restrict__ part) {
     __shared__ double s_a[RED_BT / 32], s_b[RED_BT / 32];
     double a = 0.0, b = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * RED_BT + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_BT) {
-        a += vx[i] * vx[i] + vy[i] * vy[i] + vz[i] * vz[i];
+        double ux = vx[i], uy = vy[i], uz = vz[i];
+        if (f) {                                             // the step's second half-kick, fused (as k_kick, bit for bit)
+            ux = __fma_rn(hk, f[i], ux); uy = __fma_rn(hk, f[n + i], uy); uz = __fma_rn(hk, f[2 * n + i], uz);
+            vx[i] = ux; vy[i] = uy; vz[i] = uz;
+        }
+        a += ux * ux + uy * uy + uz * uz;
         b += W[i] + W[4 * n + i] + W[8 * n + i];
     }
     for (int d = 16; d > 0; d >>= 1) { a += __shfl_down_sync(0xffffffffu, a, d); b += __shfl_down_sync(0xffffffffu, b, d); }
@@ -43,10 +48,11 @@ __global__ void k_npt_scale(int64_t n, double* __restrict__ x, double* __restric
 }  // namespace
 
 // sum v^2 and tr sum W -> HOST out[2]; synchronises the stream
-int md_launch_npt_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,
-                       const double* W, double out[2], cudaStream_t s) {
+// f != nullptr: v += hk f first (the velocity-Verlet kick that ends the step), in the same pass
+int md_launch_npt_sums(md_neighbors* nl, int64_t n, double* vx, double* vy, double* vz,
+                       const double* W, const double* f, double hk, double out[2], cudaStream_t s) {
     ProfScope prof(nl, MD_KIND_INTEGRATE, 2, s);
-    k_npt_partial<<<RED_BLOCKS, RED_BT, 0, s>>>(n, vx, vy, vz, W, nl->npt_part);
+    k_npt_partial<<<RED_BLOCKS, RED_BT, 0, s>>>(n, vx, vy, vz, W, f, hk, nl->npt_part);
     k_npt_final<<<1, 32, 0, s>>>(nl->npt_part, nl->npt_part + 2 * RED_BLOCKS);
     MD_CUDA_TRY(cudaMemcpyAsync(nl->h_npt, nl->npt_part + 2 * RED_BLOCKS, 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
     MD_CUDA_TRY(cudaStreamSynchronize(s));
