@@ -33,3 +33,21 @@ def test_heat_current_series_matches_oracle(pot):
         assert np.abs(st[k] - ref[k]).max() <= 1e-11, k
     kap = green_kubo.running_kappa(Jp + Jk, 3.0, 600.0, float(np.prod(s["box"])), 4)
     assert kap.shape == (4,) and kap[0] == 0.0 and np.isfinite(kap).all()
+
+
+def test_heat_run_is_the_nve_trajectory_with_trailing_partial_segment():
+    """25 steps sampled every 10th: two samples, and a trailing segment of 5 steps without one; the state must be
+    bit for bit that of md_nve_run over the same 25 steps (the sampling only reads), also across the rebuilds."""
+    s = mi.silicon_crystal(4, 0.05, 300.0, 5)
+    p = mi.TERSOFF_SI_C
+    a, b = GpuSystem(s, 16), GpuSystem(s, 16)
+    fa = torch.zeros((3, a.n), dtype=torch.float64, device=DEV)
+    fb = torch.zeros((3, b.n), dtype=torch.float64, device=DEV)
+    Jp, Jk = md.md_nve_heat_run(a.nl, "tersoff", p, a.n, a.x, a.y, a.z, a.vx, a.vy, a.vz, fa, False, a.box, a.mass,
+                                1.0, 25, 10, 3.5, 10)
+    md.md_nve_run(b.nl, "tersoff", p, b.n, b.x, b.y, b.z, b.vx, b.vy, b.vz, fb, False, None, b.box, b.mass, 1.0, 25,
+                  10, 3.5)
+    md.md_neighbors_status(a.nl); md.md_neighbors_status(b.nl)
+    assert len(Jp) == 2 and len(Jk) == 2
+    for u, v in ((a.x, b.x), (a.y, b.y), (a.z, b.z), (a.vx, b.vx), (a.vy, b.vy), (a.vz, b.vz), (fa, fb)):
+        assert torch.equal(u, v)
