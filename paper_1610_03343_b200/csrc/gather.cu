@@ -40,7 +40,7 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
     if (i0 >= n) return;
     T hx[4], hy[4], hz[4];
 #pragma unroll
-    for (int sl = 0; sl < 4; ++sl) rm::load_rec(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
+    for (int sl = 0; sl < 4; ++sl) rm::load_rec_once(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
     unsigned long long mask = MASK[i];
     // own halves the pair kernel left (read-modify-write at the end): requested now, not after the arithmetic
     double of[3] = {0, 0, 0}, ow[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -101,7 +101,7 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
             const int m = __ffsll((long long)run) - 1;
             run &= run - 1;
             T px, py, pz;
-            rm::load_rec(&Q[(int64_t)sl * n + i], &px, &py, &pz);
+            rm::load_rec_once(&Q[(int64_t)sl * n + i], &px, &py, &pz);
             Fx += px; Fy += py; Fz += pz;
             if (GEOM) {
                 const int j = NL[(int64_t)m * n + i];
@@ -114,7 +114,7 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
             const int m = __ffsll((long long)mask) - 1;
             mask &= mask - 1;
             T px, py, pz;
-            rm::load_rec(&Q[(int64_t)m * n + i], &px, &py, &pz);
+            rm::load_rec_once(&Q[(int64_t)m * n + i], &px, &py, &pz);
             Fx += px; Fy += py; Fz += pz;
             if (GEOM) {
                 const int j = NL[(int64_t)m * n + i];
@@ -161,9 +161,9 @@ k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int 
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T hx[4], hy[4], hz[4];
 #pragma unroll
-    for (int sl = 0; sl < 4; ++sl) rm::load_rec(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
-    unsigned long long mask = MASK[i];
-    const double ox = f[i], oy = f[n + i], oz = f[2 * n + i];           // own halves sum_j P_ij
+    for (int sl = 0; sl < 4; ++sl) rm::load_rec_once(&Q[(int64_t)(sl < K ? sl : 0) * n + i], &hx[sl], &hy[sl], &hz[sl]);
+    unsigned long long mask = rm::load_once(&MASK[i]);
+    const double ox = rm::load_once(&f[i]), oy = rm::load_once(&f[n + i]), oz = rm::load_once(&f[2 * n + i]);   // own halves sum_j P_ij
     if (dense) {                                             // popc(mask) consecutive slots
         const int cnt = __popcll(mask);
 #pragma unroll
@@ -172,7 +172,7 @@ k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int 
         for (int s0 = 4; s0 < cnt; s0 += 4) {                // the rest four at a time: loads first, sums in slot order
 #pragma unroll
             for (int u = 0; u < 4; ++u)
-                rm::load_rec(&Q[(int64_t)(s0 + u < cnt ? s0 + u : s0) * n + i], &hx[u], &hy[u], &hz[u]);
+                rm::load_rec_once(&Q[(int64_t)(s0 + u < cnt ? s0 + u : s0) * n + i], &hx[u], &hy[u], &hz[u]);
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 if (s0 + u < cnt) { Fx += hx[u]; Fy += hy[u]; Fz += hz[u]; }
@@ -186,7 +186,7 @@ k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int 
             const int m = __ffsll((long long)mask) - 1;
             mask &= mask - 1;
             T qx, qy, qz;
-            rm::load_rec(&Q[(int64_t)m * n + i], &qx, &qy, &qz);
+            rm::load_rec_once(&Q[(int64_t)m * n + i], &qx, &qy, &qz);
             Fx += qx; Fy += qy; Fz += qz;
         }
     }
