@@ -141,7 +141,10 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
 #define MD_GVV_BT 128
 #endif
 template <class T, class Rec, int MODE>
-__global__ void __launch_bounds__(MD_GVV_BT, 1024 / MD_GVV_BT)
+#ifndef MD_GVV_CPS
+#define MD_GVV_CPS 4          // no tighter register cap: 8 CTAs per SM (64 registers) cost a spill and 1 %
+#endif
+__global__ void __launch_bounds__(MD_GVV_BT, MD_GVV_CPS)
 k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int dense,   // Q, MASK, f: no __restrict__/.nc --
             double* f, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,   // the pair kernel
             double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,           // before wrote them

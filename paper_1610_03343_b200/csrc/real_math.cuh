@@ -47,15 +47,17 @@ __device__ __forceinline__ void load_rec(const PairRec64* q, double* px, double*
 // velocities and list rows of the next pair kernel out of the 126 MB L2 (config 2: 0.0687 -> 0.0650 ms per step,
 // the fused gather 22.7 -> 19.2 us; SW 0.1895 -> 0.1821).
 __device__ __forceinline__ void load_rec_once(const PairRec64* q, double* px, double* py, double* pz) {
-    double a, b, c, d;
+    double a, b, c;
+    [[maybe_unused]] double d;
     asm volatile("ld.global.cs.v2.f64 {%0,%1}, [%2];" : "=d"(a), "=d"(b) : "l"(q));
     asm volatile("ld.global.cs.v2.f64 {%0,%1}, [%2];" : "=d"(c), "=d"(d) : "l"(reinterpret_cast<const double2*>(q) + 1));
-    *px = a; *py = b; *pz = c; (void)d;
+    *px = a; *py = b; *pz = c;
 }
 __device__ __forceinline__ void load_rec_once(const float4* q, float* px, float* py, float* pz) {
-    float a, b, c, d;
+    float a, b, c;
+    [[maybe_unused]] float d;
     asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a), "=f"(b), "=f"(c), "=f"(d) : "l"(q));
-    *px = a; *py = b; *pz = c; (void)d;
+    *px = a; *py = b; *pz = c;
 }
 __device__ __forceinline__ double load_once(const double* p) {
     double v;
