@@ -44,10 +44,10 @@ k_gather(int64_t n, int K, const double* __restrict__ x, const double* __restric
     unsigned long long mask = MASK[i];
     // own halves the pair kernel left (read-modify-write at the end): requested now, not after the arithmetic
     double of[3] = {0, 0, 0}, ow[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-    if (f) { of[0] = f[i]; of[1] = f[n + i]; of[2] = f[2 * n + i]; }
+    if (f) { of[0] = rm::load_once(&f[i]); of[1] = rm::load_once(&f[n + i]); of[2] = rm::load_once(&f[2 * n + i]); }
     if (GEOM && virial) {
 #pragma unroll
-        for (int q = 0; q < 9; ++q) ow[q] = virial[(int64_t)q * n + i];
+        for (int q = 0; q < 9; ++q) ow[q] = rm::load_once(&virial[(int64_t)q * n + i]);
     }
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
