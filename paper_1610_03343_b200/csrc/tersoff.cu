@@ -31,8 +31,11 @@ template <class T> struct TsPair { T A, B, lambda, mu, R, w, chi; };     // w = 
 template <class T> struct TsCenter { T beta, n, h, c2, d2, c2_over_d2, minus_half_over_n; };
 template <class T, int NT> struct TersoffTab { TsCenter<T> c[NT]; TsPair<T> p[NT * NT]; };
 
-#ifndef LEAN_DEBUG_SLOW
-#define LEAN_DEBUG_SLOW false
+// Validation build (-DMD_TERSOFF_ALL_GENERAL=true through MD_NVCC_EXTRA): every atom of the crystal kernels takes
+// the warp-per-atom general path, so the full-size parity tests exercise it on all 512 000 atoms, not on the
+// handful that need it (done once per change of that path; profiles/r02_general_path_validation.md).
+#ifndef MD_TERSOFF_ALL_GENERAL
+#define MD_TERSOFF_ALL_GENERAL false
 #endif
 #ifndef MD_TERSOFF_LEAN_BT
 #define MD_TERSOFF_LEAN_BT 128
@@ -545,7 +548,7 @@ k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double*
     const ps::MinImage mi = ps::make_min_image(Lx, Ly, Lz);
     T ex[MR], ey[MR], ez[MR], d2[MR];
     unsigned mask = 0u;
-    bool slow = nn > MR || LEAN_DEBUG_SLOW;
+    bool slow = nn > MR || MD_TERSOFF_ALL_GENERAL;
     {
         bool far = false;
 #pragma unroll
