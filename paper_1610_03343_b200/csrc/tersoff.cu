@@ -598,7 +598,7 @@ tersoff_binned_cta(int64_t cta, int64_t n, const double* __restrict__ x, const d
                    double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial) {
     const int64_t cnt = *count;
     const int64_t t0 = cta * BT + threadIdx.x;
-    if (t0 >= cnt) return;                                   // no barrier follows
+    if (t0 >= cnt) return;                                   // no barrier follows (the caller may still wait on the grid)
     const int64_t i = list[t0];
     unsigned long long run = MASK[i];
     const int M = min(__popcll(run), MR);
@@ -877,6 +877,29 @@ k_tersoff_hot(int64_t n, int tail_ctas, const double* __restrict__ x, const doub
                                            counts, p, tb, Q, MASK, pe, f, virial);
 }
 
+// The bin with at most MR in-range neighbours as a kernel of its own (k_tersoff_hot_tail, the loop code on the small
+// tail bin, is launched just before it).  It needs nothing from that kernel, so it is launched as its programmatic
+// dependent and does NOT wait at its start: both run side by side from the first cycle, the tail's few long-latency
+// CTAs with their 52-68 KB of shared memory on some SMs, this kernel -- a few KB of shared memory, the whole L1 for
+// its gathers -- everywhere else.  Its last `wait_ctas` CTAs call griddepcontrol.wait when their work is done, so
+// that "this grid has completed" implies "the tail kernel has completed" for whatever follows on the stream; they
+// are dispatched last, long after the tail kernel has finished, and never actually wait.
+template <class T, class Rec, int MR, int BT, int MAXREG>
+__global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
+k_tersoff_binned(int64_t n, int wait_ctas, const double* __restrict__ x, const double* __restrict__ y,
+                 const double* __restrict__ z, double Lx, double Ly, double Lz,
+                 const int32_t* __restrict__ NL, const uint8_t* __restrict__ REV, TersoffDev<T> p,
+                 const int32_t* list, const int32_t* count, const double* __restrict__ gtab, Rec* __restrict__ Q,
+                 const unsigned long long* MASK, double* __restrict__ pe, double* __restrict__ f,
+                 double* __restrict__ virial) {
+    __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
+    const fm::Tab tb = fm::stage_tables(s_tab, gtab);
+    md_grid_release();
+    __syncthreads();
+    tersoff_binned_cta<T, Rec, MR, BT>(blockIdx.x, n, x, y, z, Lx, Ly, Lz, NL, REV, list, count, p, tb, Q, MASK, pe, f, virial);
+    if ((int)blockIdx.x >= (int)gridDim.x - wait_ctas) md_grid_wait();
+}
+
 template <class T>
 TersoffDev<T> make_dev(const md_tersoff_params* hp) {
     TersoffDev<T> p;
@@ -926,7 +949,7 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
     int32_t* const counts = nl->bin_count + 4 * nl->bin_phase;   // (zeroed by this k_screen, see pair_sort.cuh)
     bins.count = counts;
     bins.count_next = NT == 1 ? nl->bin_count + 4 * (nl->bin_phase ^ 1) : nullptr;
-    nl->launches[MD_KIND_PAIR] += NT == 1 ? 2 : 1;
+    nl->launches[MD_KIND_PAIR] += NT == 1 ? (sizeof(T) == 8 ? 3 : 2) : 1;
     MD_CUDA_TRY(md_launch_pdl(ps::k_screen<T>, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, s, pdl, (unsigned)n, x, y, z,
                               box[0], box[1], box[2], nl->NN, nl->NL, rt, NT > 1 ? types : (const int32_t*)nullptr, nl->MASK, bins));
     nl->q_dense = 1;
@@ -940,14 +963,31 @@ int launch_sorted(md_neighbors* nl, int64_t n, const double* x, const double* y,
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if constexpr (NT == 1) {
-        const int tail = sms;                                // one loop-code CTA per SM for the tail bin
-        auto hot = k_tersoff_hot<T, Rec, 4, BT, PCA, 168>;
-        const int rch = md_allow_dynamic_smem((const void*)hot, (int)sizeof(Sm));
-        if (rch != MD_OK) return rch;
-        MD_CUDA_TRY(md_launch_pdl(hot, dim3(grid + (unsigned)tail), dim3(BT), sizeof(Sm), s, true, n, tail, x, y, z, box[0],
-                                  box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, (const int32_t*)nl->bin_list,
-                                  (const int32_t*)counts, gtab, (Rec*)nl->Q, (const unsigned long long*)nl->MASK, pe, f,
-                                  virial, nl->d_status));
+        const int tail = sms;                                // loop-code CTAs for the tail bin, striding over its tiles
+        if constexpr (sizeof(T) == 8) {
+            // FP64: tail bin first, then the register kernel beside it as a dependent that does not wait
+            // (k_tersoff_binned): without the tail's 68 KB shared-memory pool in every CTA the register body has the
+            // whole L1 for its gathers and fits 4 CTAs per SM at 128 registers (0.1244 -> 0.1140 ms per step on config 5)
+            MD_CUDA_TRY(md_launch_pdl(kern, dim3((unsigned)tail), dim3(BT), sizeof(Sm), s, true, n, x, y, z, box[0], box[1],
+                                      box[2], nl->NN, nl->NL, nl->REV, p, tab, (const int32_t*)nullptr,
+                                      (const int32_t*)(nl->bin_list + 2 * n), (const int32_t*)(counts + 2), gtab, (Rec*)nl->Q,
+                                      (const unsigned long long*)nl->MASK, pe, f, virial, nl->d_status));
+            MD_CUDA_TRY(md_launch_pdl(k_tersoff_binned<T, Rec, 4, BT, 128>, dim3(grid), dim3(BT), 0, s, true, n, sms, x, y, z,
+                                      box[0], box[1], box[2], nl->NL, nl->REV, p, (const int32_t*)nl->bin_list,
+                                      (const int32_t*)counts, gtab, (Rec*)nl->Q, (const unsigned long long*)nl->MASK, pe, f,
+                                      virial));
+        } else {
+            // FP32 mode: one launch, the first CTAs on the tail bin (measured: split 0.1033 / 0.0999 vs 0.0946 ms per
+            // step -- the cheap float register body leaves the tail's tiles as the critical path, and they run
+            // faster beside 2 than beside 4 register-body CTAs per SM)
+            auto hot = k_tersoff_hot<T, Rec, 4, BT, PCA, 168>;
+            const int rch = md_allow_dynamic_smem((const void*)hot, (int)sizeof(Sm));
+            if (rch != MD_OK) return rch;
+            MD_CUDA_TRY(md_launch_pdl(hot, dim3(grid + (unsigned)tail), dim3(BT), sizeof(Sm), s, true, n, tail, x, y, z, box[0],
+                                      box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, (const int32_t*)nl->bin_list,
+                                      (const int32_t*)counts, gtab, (Rec*)nl->Q, (const unsigned long long*)nl->MASK, pe, f,
+                                      virial, nl->d_status));
+        }
     } else {
         MD_CUDA_TRY(md_launch_pdl(kern, dim3(std::min<unsigned>(grid, 3u * (unsigned)sms)), dim3(BT), sizeof(Sm), s, true, n,
                                   x, y, z, box[0], box[1], box[2], nl->NN, nl->NL, nl->REV, p, tab, types,
