@@ -223,7 +223,7 @@ def kernel_name(md, nl, pot, n):
         return "k_screen+k_sw_sorted"
     _, long_rows = md.md_neighbors_row_stats(nl)
     # md_nve_run asks for no virial: the register path is the 128-register lean kernel (tersoff.cu, launch())
-    return "k_screen+k_tersoff_hot" if long_rows * 256 > n else "k_tersoff_lean"
+    return "k_screen+k_tersoff_sorted|k_tersoff_binned" if long_rows * 256 > n else "k_tersoff_lean"
 
 
 def measure_nve(gpu, md, cfg_index, steps, warmup, fp32, peaks, fp64_peak, with_e2e, sampler=None):

@@ -79,7 +79,8 @@ int md_neighbors_status(md_neighbors* nl, int* max_count_seen, void* stream);
 /* Row statistics of the current list (HOST ints, either may be NULL): the longest row and the number
  * of rows longer than 4 entries.  Waits for the last build / import on its stream to finish.  The
  * Tersoff call uses them to choose its kernel: the register kernel (k_tersoff_lean, with or without the virial
- * own half) while at most one row in 256 is longer than 4, else k_screen + k_tersoff_hot. */
+ * own half) while at most one row in 256 is longer than 4, else k_screen + the binned kernels (k_tersoff_sorted on
+ * the atoms with more than 4 in-range neighbours beside k_tersoff_binned on the others; FP32: k_tersoff_hot). */
 int md_neighbors_row_stats(md_neighbors* nl, int* max_row, int* rows_longer_than_4);
 
 /* Copy the current list out / in (DEVICE int32 buffers): NN[n]; NL[max_neighbors][n] neighbour-major,
