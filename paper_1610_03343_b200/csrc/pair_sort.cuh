@@ -166,16 +166,30 @@ k_screen(unsigned n, const double* x, const double* y, const double* z,
         bin = M <= bins.b0 ? 0 : (M <= bins.b1 ? 1 : 2);
     }
     if (!bins.list) return;
-    const unsigned lane = threadIdx.x & 31;
+    // One atomic per CTA and bin (not per warp: 16 000 warps adding to the same three counters serialise in L2):
+    // per-warp counts -> shared memory, warp 0 reserves the CTA's range of each bin, every warp takes its part.
+    // The order inside a bin's list is whatever the CTAs' atomics make it, which is harmless: what is computed for an
+    // atom does not depend on which thread computes it.
+    __shared__ int s_cnt[3][8], s_base[3][8];                // 256 threads = 8 warps
+    const unsigned lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    unsigned v[3];
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
-        const unsigned v = __ballot_sync(0xffffffffu, bin == b);
-        if (!v) continue;
-        int base = 0;
-        if (lane == (unsigned)(__ffs(v) - 1)) base = atomicAdd(&bins.count[b], __popc(v));
-        base = __shfl_sync(0xffffffffu, base, __ffs(v) - 1);
-        if (bin == b) bins.list[(size_t)b * n + base + __popc(v & ((1u << lane) - 1u))] = (int)i;
+        v[b] = __ballot_sync(0xffffffffu, bin == b);
+        if (lane == 0) s_cnt[b][wid] = __popc(v[b]);
     }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        const int b = threadIdx.x;
+        int tot = 0, off[8];
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { off[w] = tot; tot += s_cnt[b][w]; }
+        const int base = tot ? atomicAdd(&bins.count[b], tot) : 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) s_base[b][w] = base + off[w];
+    }
+    __syncthreads();
+    if (bin >= 0) bins.list[(size_t)bin * n + s_base[bin][wid] + __popc(v[bin] & ((1u << lane) - 1u))] = (int)i;
 }
 
 // Dense record layout: the record of pair (i -> j) goes to the slot of row j that counts the in-range entries
