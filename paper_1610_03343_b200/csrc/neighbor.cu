@@ -253,7 +253,7 @@ k_search(int64_t n, Grid g, const double4* sorted, const float4* sortedf,
     {   // longest row: one atomic per warp
         const unsigned act = __activemask();
         const int wmax = __reduce_max_sync(act, cnt);
-        if ((tid & 31) == __ffs(act) - 1) atomicMax(&status[1], wmax);
+        if ((tid & 31) == __ffs(act) - 1 && wmax > __ldcg(&status[1])) atomicMax(&status[1], wmax);   // 16 000 warps, one word: only a larger value goes out
     }
     NN[i] = cnt;
     for (int m = 1; m < cnt; ++m) {                          // insertion sort of the (short) row by index
@@ -289,7 +289,7 @@ k_reverse(int64_t n, int K, const int32_t* NN, const int32_t* NL,
         const int wmax = __reduce_max_sync(act, nn);
         const int nlong = __popc(__ballot_sync(act, nn > 4));
         if ((threadIdx.x & 31) == __ffs(act) - 1) {
-            atomicMax(&status[1], wmax);
+            if (wmax > __ldcg(&status[1])) atomicMax(&status[1], wmax);
             if (nlong) atomicAdd(&status[2], nlong);
         }
     }
