@@ -14,7 +14,7 @@ namespace {
 bool valid_box(const double box[3]) { return box && box[0] > 0 && box[1] > 0 && box[2] > 0; }
 
 void free_all(md_neighbors* nl) {
-    cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->Q); cudaFree(nl->MASK); cudaFree(nl->bin_list); cudaFree(nl->bin_count);
+    cudaFree(nl->NN); cudaFree(nl->NL); cudaFree(nl->REV); cudaFree(nl->HEAD); cudaFree(nl->Q); cudaFree(nl->MASK); cudaFree(nl->bin_list); cudaFree(nl->bin_count);
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e); cudaFree(nl->npt_w); cudaFree(nl->npt_part);
     if (nl->h_npt) cudaFreeHost(nl->h_npt);
@@ -151,6 +151,7 @@ int md_neighbors_create(md_neighbors** out, int64_t n_atoms, int max_neighbors) 
     ok = ok && cudaMalloc(&nl->NN, n * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->NL, n * K * sizeof(int32_t)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->REV, n * K) == cudaSuccess;
+    ok = ok && cudaMalloc(&nl->HEAD, n * sizeof(MdRowHead)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->Q, n * K * sizeof(PairRec64)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->MASK, n * sizeof(unsigned long long)) == cudaSuccess;
     ok = ok && cudaMalloc(&nl->bin_list, 3 * n * sizeof(int32_t)) == cudaSuccess;

@@ -26,6 +26,9 @@ enum : int {
 // FP32 mode stores float4 in the first 16 bytes of a 16-byte-strided array.
 struct __align__(32) PairRec64 { double x, y, z, w; };
 
+// Head of a list row for the crystal pair kernel: first four entries, their reverse slots, the row length (32 bytes).
+struct __align__(32) MdRowHead { int j[4]; unsigned rev; int nn; int pad[2]; };
+
 struct md_neighbors {
     int64_t n_cap;          // capacity in atoms
     int64_t n;              // atoms of the current list (0 = none)
@@ -34,6 +37,7 @@ struct md_neighbors {
     int32_t* NN;            // [n]
     int32_t* NL;            // [K][n] neighbour-major
     uint8_t* REV;           // [K][n] position of i in row NL[m][i]
+    MdRowHead* HEAD;        // [n] the first four entries of each row with their reverse slots (k_reverse writes it)
     // per-pair records, pushed layout: Q[m*n + i] = P_{j i}, j = NL[m][i]
     void* Q;                // K*n*32 bytes
     unsigned long long* MASK;  // [n] bit m set <=> slot m is inside the force range

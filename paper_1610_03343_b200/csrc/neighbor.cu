@@ -278,7 +278,7 @@ k_search(int64_t n, Grid g, const double4* sorted, const float4* sortedf,
 template <bool CHECK>
 __global__ void __launch_bounds__(128)
 k_reverse(int64_t n, int K, const int32_t* NN, const int32_t* NL,
-          uint8_t* __restrict__ REV, int* __restrict__ status) {
+          uint8_t* __restrict__ REV, int* __restrict__ status, MdRowHead* __restrict__ HEAD) {
     md_grid_wait();
     md_grid_release();
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -348,7 +348,17 @@ k_reverse(int64_t n, int K, const int32_t* NN, const int32_t* NL,
             }
             REV[(int64_t)(m0 + u) * n + i] = (uint8_t)lo[u];
         }
+        if (m0 == 0) {
+            // the row's head as ONE 32-byte record for the crystal pair kernel (k_tersoff_lean): its first four
+            // entries, their reverse slots (one byte each) and the row length
+            MdRowHead hd;
+            hd.j[0] = j[0]; hd.j[1] = j[1]; hd.j[2] = j[2]; hd.j[3] = j[3];
+            hd.rev = (unsigned)lo[0] | (unsigned)lo[1] << 8 | (unsigned)lo[2] << 16 | (unsigned)lo[3] << 24;
+            hd.nn = nn; hd.pad[0] = hd.pad[1] = 0;
+            HEAD[i] = hd;
+        }
     }
+    if (nn == 0) { MdRowHead hd = {{0, 0, 0, 0}, 0u, 0, {0, 0}}; HEAD[i] = hd; }
 }
 
 }  // namespace
@@ -358,9 +368,9 @@ int md_launch_reverse(md_neighbors* nl, cudaStream_t s, int check) {
     if (n == 0) return MD_OK;
     ProfScope prof(nl, MD_KIND_BUILD, 1, s);
     // after k_search (a build) as a programmatic dependent; after the copies of an import as a normal launch
-    if (check) k_reverse<true><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status);
+    if (check) k_reverse<true><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, nl->K, nl->NN, nl->NL, nl->REV, nl->d_status, nl->HEAD);
     else MD_CUDA_TRY(md_launch_pdl(k_reverse<false>, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, s, true, n, nl->K, nl->NN,
-                                   nl->NL, nl->REV, nl->d_status));
+                                   nl->NL, nl->REV, nl->d_status, nl->HEAD));
     MD_CUDA_TRY(cudaGetLastError());
     MD_CUDA_TRY(cudaMemcpyAsync(nl->h_maxrow, nl->d_status + 1, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     MD_CUDA_TRY(cudaEventRecord(nl->ev_list, s));

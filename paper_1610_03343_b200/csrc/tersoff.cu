@@ -515,23 +515,27 @@ __global__ void __launch_bounds__(BT) __maxnreg__(MAXREG)
 k_tersoff_lean(int64_t n, int K, const double* x, const double* y, const double* z,   // no __restrict__ (see the wait below)
                double Lx, double Ly, double Lz,
                const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-               const uint8_t* __restrict__ REV, TersoffDev<T> p, const double* __restrict__ gtab,
-               Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
+               const uint8_t* __restrict__ REV, const MdRowHead* __restrict__ HEAD, TersoffDev<T> p,
+               const double* __restrict__ gtab, Rec* __restrict__ Q, unsigned long long* __restrict__ MASK,
                double* __restrict__ pe, double* __restrict__ f, double* __restrict__ virial, int* __restrict__ status) {
+    static_assert(MR == 4, "the row head record holds four entries");
     __shared__ __align__(16) double s_tab[fm::TAB_DOUBLES];
     __shared__ SlowQueue<T, BT> s_slow;
     if (threadIdx.x == 0) { s_slow.count = 0; s_slow.p = p; }
     const int64_t i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t i = i0 < n ? i0 : n - 1;
-    const int nn = NN[i];
+    // the row's first four entries, their reverse slots and its length: one 32-byte record (k_reverse wrote it)
+    int4 h0; unsigned hrev; int nn;
+    asm volatile("ld.global.nc.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(h0.x), "=r"(h0.y), "=r"(h0.z), "=r"(h0.w) : "l"(HEAD + i));
+    asm volatile("ld.global.nc.v2.b32 {%0,%1}, [%2];" : "=r"(hrev), "=r"(nn) : "l"(reinterpret_cast<const int*>(HEAD + i) + 4));
+    const int hj[4] = {h0.x, h0.y, h0.z, h0.w};
     int jd[MR];
     unsigned qi[MR];
 #pragma unroll
     for (int m = 0; m < MR; ++m) {
-        const int mk = m < K ? m : 0;
-        const int jr = NL[(int64_t)mk * n + i];
+        const int jr = hj[m];
         jd[m] = (unsigned)jr < (unsigned long long)n ? jr : (int)i;
-        qi[m] = (unsigned)REV[(int64_t)mk * n + i] * (unsigned)n + (unsigned)jd[m];   // n * K <= 2e9 (md_neighbors_create)
+        qi[m] = (hrev >> (8 * m) & 255u) * (unsigned)n + (unsigned)jd[m];   // n * K <= 2e9 (md_neighbors_create)
     }
     const fm::Tab tb = fm::stage_tables(s_tab, gtab);
     // Inside md_nve_run this kernel is launched as a programmatic dependent of the fused gather kernel that
@@ -1025,11 +1029,11 @@ int launch(md_neighbors* nl, int64_t n, const double* x, const double* y, const 
         if (virial)
             MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG, true>, dim3((unsigned)((n + LBT - 1) / LBT)),
                                       dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
-                                      nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
+                                      nl->REV, (const MdRowHead*)nl->HEAD, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
         else
             MD_CUDA_TRY(md_launch_pdl(k_tersoff_lean<T, Rec, 4, LBT, MD_TERSOFF_LEAN_MAXREG, false>, dim3((unsigned)((n + LBT - 1) / LBT)),
                                       dim3(LBT), 0, s, pdl, n, nl->K, x, y, z, box[0], box[1], box[2], nl->NN, nl->NL,
-                                      nl->REV, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
+                                      nl->REV, (const MdRowHead*)nl->HEAD, p, gtab, (Rec*)nl->Q, nl->MASK, pe, f, virial, nl->d_status));
         nl->gather_pdl = 1;
         return MD_OK;
     }
