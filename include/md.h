@@ -50,7 +50,8 @@ typedef enum {
     MD_ERR_NEIGHBOR_OVERFLOW = -4,   /* a row needs more than max_neighbors entries */
     MD_ERR_CUDA = -5,
     MD_ERR_NO_LIST = -6,             /* force call before a list was built or imported */
-    MD_ERR_LIST_ASYMMETRIC = -7      /* j in row i but i not in row j (imported list) */
+    MD_ERR_LIST_ASYMMETRIC = -7,     /* j in row i but i not in row j (imported list) */
+    MD_ERR_STATIC_CAPACITY = -8      /* md_tersoff_force_static: n * max_neighbors > MD_STATIC_MAX_PAIRS */
 } md_status;
 
 enum { MD_FP64 = 0, MD_FP32 = 1 };          /* arithmetic of the force kernels (reading A10) */
@@ -217,6 +218,32 @@ int md_profile_read(md_neighbors* nl, double* ms, int64_t* launches);
  * force range, out[2] = ordered in-range triplets sum_i M_i (M_i - 1).  bench.py multiplies them by the
  * per-unit operation counts of DESIGN.md section 3 to get the algorithmic work of a launch.  Synchronous. */
 int md_pair_counts(md_neighbors* nl, int64_t out[3], void* stream);
+
+/* Tersoff energies and forces for callers that may not allocate (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the stored-P scheme of steps 2+3 (P_ij = dU_i/dr_ij per listed pair, Eq. 14 at
+ * PAPER.md:173-176; F_i = sum_j (P_ij - P_ji), Eq. 28 at PAPER.md:330) with its per-pair records in a fixed
+ * file-scope device array of the library instead of a handle: 32 bytes x MD_STATIC_MAX_PAIRS + 256 bytes = 16 MiB,
+ * held by every GPU that loads the library until the process exits.  The call needs no md_neighbors handle and calls
+ * no cudaMalloc, cudaFree or allocating library routine; FP64 arithmetic, the same formulas and device functions as
+ * md_tersoff_force.
+ *   n, max_neighbors: n * max_neighbors <= MD_STATIC_MAX_PAIRS, else MD_ERR_STATIC_CAPACITY (nothing is enqueued);
+ *       1 <= max_neighbors <= MD_MAX_NEIGHBORS.
+ *   NN[n], NL[max_neighbors][n] (DEVICE int32): the list in the layout of md_neighbors_export; it must be symmetric
+ *       (j in row i <=> i in row j).  Rows need not be sorted.
+ *   x, y, z (DEVICE), box (HOST double[3]): coordinates in [0, box[a]), minimum image, box[a] >= 2 S.
+ *   pe[n], f[3][n] (DEVICE, either may be NULL): U_i and F_i.
+ *   status (DEVICE int32*, may be NULL): receives 0, or bit 0 (1) = some NN[i] > max_neighbors (row clamped),
+ *       bit 1 (2) = some listed j has no entry i in its own row (F of that atom is NaN) or is
+ *       outside [0, n) (the row ends there); written on `stream`.
+ * Every call on a device shares the one array, and the array keeps the last call's contents: each call clears its
+ * status word and writes every record before reading it, so calls on ONE stream (or ordered by events) are
+ * independent of each other, but two calls that overlap on the GPU (two streams, two host threads) race and give
+ * wrong results.  The first call on a device looks the array's address up (cudaGetSymbolAddress, loads the
+ * module): make it outside stream capture.  Asynchronous like the other force calls. */
+enum { MD_STATIC_MAX_PAIRS = 524288 };
+int md_tersoff_force_static(int64_t n, int max_neighbors, const int32_t* NN, const int32_t* NL,
+                            const double* x, const double* y, const double* z, const double box[3],
+                            const md_tersoff_params* p, double* pe, double* f, int32_t* status, void* stream);
 
 /* Library version string (HOST, static storage). */
 const char* md_version(void);

@@ -14,12 +14,14 @@ from . import build as _build
 MD_OK = 0
 MD_ERR_ARG, MD_ERR_ALLOC, MD_ERR_BOX_TOO_SMALL, MD_ERR_NEIGHBOR_OVERFLOW = -1, -2, -3, -4
 MD_ERR_CUDA, MD_ERR_NO_LIST, MD_ERR_LIST_ASYMMETRIC = -5, -6, -7
+MD_ERR_STATIC_CAPACITY = -8
 MD_FP64, MD_FP32 = 0, 1
 MD_TERSOFF, MD_SW = 0, 1
 MD_MAX_NEIGHBORS = 64
+MD_STATIC_MAX_PAIRS = 524288
 
 _ERR = {-1: "MD_ERR_ARG", -2: "MD_ERR_ALLOC", -3: "MD_ERR_BOX_TOO_SMALL", -4: "MD_ERR_NEIGHBOR_OVERFLOW",
-        -5: "MD_ERR_CUDA", -6: "MD_ERR_NO_LIST", -7: "MD_ERR_LIST_ASYMMETRIC"}
+        -5: "MD_ERR_CUDA", -6: "MD_ERR_NO_LIST", -7: "MD_ERR_LIST_ASYMMETRIC", -8: "MD_ERR_STATIC_CAPACITY"}
 
 
 class MDError(RuntimeError):
@@ -44,7 +46,8 @@ EXPORTS = ("md_version", "md_neighbors_create", "md_neighbors_destroy", "md_neig
            "md_neighbors_export", "md_neighbors_import", "md_build_neighbors", "md_tersoff_force",
            "md_sw_force", "md_velocity_verlet_step", "md_nve_run", "md_nve_run_host", "md_probe_fp64_peak",
            "md_profile_enable", "md_profile_read", "md_math_probe", "md_neighbors_row_stats", "md_pair_counts",
-           "md_tersoff_multi_force", "md_tersoff_force_literal", "md_npt_run", "md_nve_heat_run")
+           "md_tersoff_multi_force", "md_tersoff_force_literal", "md_npt_run", "md_nve_heat_run",
+           "md_tersoff_force_static")
 
 _lib = None
 
@@ -178,6 +181,15 @@ def md_tersoff_force_literal(nl, n, x, y, z, vx, vy, vz, box, params, precision=
     _check(load().md_tersoff_force_literal(nl._h, C.c_int64(n), _ptr(x), _ptr(y), _ptr(z), _ptr(vx), _ptr(vy),
                                            _ptr(vz), _box(box), C.byref(p), C.c_int(precision), _ptr(pe), _ptr(f),
                                            _ptr(virial), _ptr(heat), _stream(stream)), "md_tersoff_force_literal")
+
+
+def md_tersoff_force_static(n, max_neighbors, NN, NL, x, y, z, box, params, pe=None, f=None, status=None, stream=None):
+    """Tersoff U_i and F_i with the pair records in the library's fixed device array: no handle, no allocation.
+    n * max_neighbors <= MD_STATIC_MAX_PAIRS; calls that overlap on one GPU race on the array (md.h)."""
+    p = tersoff_params(params)
+    _check(load().md_tersoff_force_static(C.c_int64(n), C.c_int(max_neighbors), _ptr(NN), _ptr(NL), _ptr(x), _ptr(y),
+                                          _ptr(z), _box(box), C.byref(p), _ptr(pe), _ptr(f), _ptr(status),
+                                          _stream(stream)), "md_tersoff_force_static")
 
 
 def tersoff_multi_params(elements, chi) -> md_tersoff_multi_params:
