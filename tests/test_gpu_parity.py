@@ -180,6 +180,40 @@ def test_dimer_and_isolated_atoms_zeta_zero_path():
         assert (out["f"][:, 2] == 0).all() and out["pe"][2] == 0
 
 
+def test_bent_trimers_and_skew_dimers_all_outputs():
+    """The clusters of tests/test_oracle_peratom_pins.py (closed-form pins of the oracle's per-atom U, F, W, J)
+    through the CUDA path: a central atom with two ends out of each other's range, bonds below R, inside the
+    cut-off window, near the SW cut-off; vacuum-padded non-cubic box; n = 3 (one ragged CTA)."""
+    def unit(theta, phi):
+        return np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    v = np.array([[0.31, -0.72, 0.23], [-0.44, 0.15, 0.61], [0.08, 0.52, -0.37]])
+    box = np.array([60.0, 55.0, 50.0])
+    cases = [("tersoff", 2.30, 2.45, 100.0), ("tersoff", 2.35, 2.85, 112.0), ("tersoff", 2.78, 2.93, 95.0),
+             ("sw", 2.30, 2.45, 140.0), ("sw", 2.20, 3.10, 150.0), ("tersoff", 2.35, None, 0.0), ("sw", 3.2, None, 0.0)]
+    for pot, r1, r2, ang in cases:
+        u1 = unit(0.7, 1.9)
+        c0 = np.array([20.3, 21.7, 19.1])
+        pos = [c0, c0 + r1 * u1]
+        if r2 is not None:
+            ax = np.cross(u1, np.array([0.2, -0.5, 0.84])); ax /= np.linalg.norm(ax)
+            a = np.deg2rad(ang)
+            u2 = u1 * np.cos(a) + np.cross(ax, u1) * np.sin(a) + ax * np.dot(ax, u1) * (1 - np.cos(a))
+            pos.append(c0 + r2 * u2)
+        pos = np.stack(pos)
+        n = pos.shape[0]
+        s = {"x": pos[:, 0].copy(), "y": pos[:, 1].copy(), "z": pos[:, 2].copy(), "box": box,
+             "vx": v[:n, 0].copy(), "vy": v[:n, 1].copy(), "vz": v[:n, 2].copy()}
+        g = GpuSystem(s, KMAX[pot])
+        g.build(mi.r_list(pot))
+        out = g.force(pot, PARAMS[pot])
+        NN, NL = oracle.neighbors(s["x"], s["y"], s["z"], box, mi.r_list(pot), KMAX[pot])
+        ref = oracle.evaluate(pot, PARAMS[pot], s["x"], s["y"], s["z"], box, NN, NL,
+                              v=(s["vx"], s["vy"], s["vz"]), precision="f80")
+        assert_close_energy(out["pe"], ref["pe"])
+        for k in ("f", "virial", "heat"):
+            assert_close_fp64(f"{pot} {r1} {r2} {k}", out[k], ref[k])
+
+
 def test_perfect_lattice_zero_force():
     x, y, z, L = mi.diamond_lattice(4)
     s = {"x": x, "y": y, "z": z, "box": np.array([L, L, L])}
