@@ -721,104 +721,179 @@ tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, 
                     d2s[u] = ps::in_range_d2((T)dx[u], (T)dy[u], (T)dz[u]);
                 }
             }
+            // both slots step by step, branch-free (a slot past the last one computes on d2 = 1 and is not stored)
+            bool val[2], win[2];
+            int tj[2];
+            T ri[2], r[2], ea[2], eb[2], fr[2], fa[2], c[2], cp[2];
+            TsPair<T> pp[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) { val[u] = k0 + u < M; d2s[u] = val[u] ? d2s[u] : T(1); }
+            fm::rsqrt_v<2>(d2s, ri);
+            bool anywin = false;
 #pragma unroll
             for (int u = 0; u < 2; ++u) {
-                if (k0 + u >= M) continue;
-                const T tx = (T)dx[u], ty = (T)dy[u], tz = (T)dz[u];
-                const T d2 = d2s[u];
-                const T ri = fm::rsqrt(d2);
-                const T r = d2 * ri;
-                const int tj = NT > 1 ? types[j[u]] : 0;
-                const TsPair<T> pp = tab.p[ti * NT + tj];    // mixed parameters of the pair (reading A17)
-                T c = T(1), cp = T(0);
-                if (r > pp.R) {                              // f_C window R < r < S (reading A1)
+                r[u] = d2s[u] * ri[u];
+                tj[u] = NT > 1 ? types[j[u]] : 0;
+                pp[u] = tab.p[ti * NT + tj[u]];              // mixed parameters of the pair (reading A17)
+                ea[u] = -pp[u].lambda * r[u]; eb[u] = -pp[u].mu * r[u];
+                win[u] = val[u] && r[u] > pp[u].R;           // f_C window R < r < S (reading A1)
+                anywin = anywin || win[u];
+                c[u] = T(1); cp[u] = T(0);
+            }
+            fm::exp_v<2>(ea, fr, tb);
+            fm::exp_v<2>(eb, fa, tb);
+            if (anywin) {
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    if (!win[u]) continue;
                     T sn, cs;
-                    fm::sincos_0_pi((r - pp.R) * pp.w, &sn, &cs);
-                    c = T(0.5) + T(0.5) * cs;
-                    cp = T(-0.5) * pp.w * sn;
+                    fm::sincos_0_pi((r[u] - pp[u].R) * pp[u].w, &sn, &cs);
+                    c[u] = T(0.5) + T(0.5) * cs;
+                    cp[u] = T(-0.5) * pp[u].w * sn;
                 }
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                if (!val[u]) continue;
                 const int q = col + 32 * (k0 + u);
-                s.ex[q] = tx * ri; s.ey[q] = ty * ri; s.ez[q] = tz * ri; s.rinv[q] = ri;
-                s.fc[q] = c; s.fcp[q] = cp;
-                s.fRD[q] = pp.A * fm::exp(-pp.lambda * r, tb);
-                s.fAh[q] = pp.chi * pp.B * fm::exp(-pp.mu * r, tb);         // chi_ij f_A: b_ij only ever multiplies it
-                s.jj[q] = j[u] | (tj << 28);                 // element of the neighbour in the top bits (n < 2^28)
+                s.ex[q] = (T)dx[u] * ri[u]; s.ey[q] = (T)dy[u] * ri[u]; s.ez[q] = (T)dz[u] * ri[u]; s.rinv[q] = ri[u];
+                s.fc[q] = c[u]; s.fcp[q] = cp[u];
+                s.fRD[q] = pp[u].A * fr[u];
+                s.fAh[q] = pp[u].chi * pp[u].B * fa[u];      // chi_ij f_A: b_ij only ever multiplies it
+                s.jj[q] = j[u] | (tj[u] << 28);              // element of the neighbour in the top bits (n < 2^28)
             }
         }
     }
 
     // pass 2: zeta_a = sum_{b != a} f_C(r_b) g_ab (Eq. 4), g in the cancellation-free form; b, b' (Eq. 3)
+    // Two slots a per iteration, every arithmetic step written for both (independent chains for the FP64 pipe;
+    // one slot at a time the kernel ran its dependent chains at ~17 cycles per instruction).  The loop over b
+    // covers all M slots and masks b == a, so both chains walk the same b; the sums keep the order b = 0..M-1.
     T U = T(0);
     // (this pass reads only e and f_C of the other slots, so D and h can replace f_R and f_A of slot a at once)
-    for (int a = 0; a < M; ++a) {
-        const int ca = col + 32 * a;
-        const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
-        T zt = T(0);
-        auto zterm = [&](int b) {
-            const int cb = col + 32 * b;
-            const T cs = ax * s.ex[cb] + ay * s.ey[cb] + az * s.ez[cb];
-            const T xx = pc.h - cs;
-            const T x2 = xx * xx;
-            zt += s.fc[cb] * (T(1) + pc.c2_over_d2 * x2 * fm::rcp(pc.d2 + x2));
-        };
-#pragma unroll 2
-        for (int b = 0; b < a; ++b) zterm(b);
-#pragma unroll 2
-        for (int b = a + 1; b < M; ++b) zterm(b);
-        T bo = T(1), bp = T(0);
-        if (zt > T(0)) {                                     // zeta = 0: b = 1, b' = 0 (reading A8)
-            const T tt = fm::exp(pc.n * fm::log(pc.beta * zt, tb), tb);             // (beta zeta)^n
-            bo = fm::exp(pc.minus_half_over_n * fm::log(T(1) + tt, tb), tb);        // Eq. (3)
-            bp = T(-0.5) * bo * tt * fm::rcp(zt * (T(1) + tt));
+    for (int a0 = 0; a0 < M; a0 += 2) {
+        int av[2], ca[2];
+        bool val[2];
+        T ax[2], ay[2], az[2], zt[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            val[u] = a0 + u < M;
+            av[u] = val[u] ? a0 + u : a0;
+            ca[u] = col + 32 * av[u];
+            ax[u] = s.ex[ca[u]]; ay[u] = s.ey[ca[u]]; az[u] = s.ez[ca[u]];
+            zt[u] = T(0);
         }
-        const T c = s.fc[ca], cp = s.fcp[ca], fR = s.fRD[ca], fA = s.fAh[ca];
-        const TsPair<T> pp = tab.p[ti * NT + (NT > 1 ? (int)((unsigned)s.jj[ca] >> 28) : 0)];
-        const T bfA = bo * fA;
-        U += T(0.5) * c * (fR - bfA);                                                  // U_ia / 2
-        s.fRD[ca] = T(0.5) * (cp * (fR - bfA) + c * (pp.mu * bfA - pp.lambda * fR));   // D
-        s.fAh[ca] = T(-0.5) * c * fA * bp;                                             // h
+#pragma unroll 2
+        for (int b = 0; b < M; ++b) {
+            const int cb = col + 32 * b;
+            const T bx = s.ex[cb], by = s.ey[cb], bz = s.ez[cb], fcb = s.fc[cb];
+            T x2[2], den[2], q[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const T cs = ax[u] * bx + ay[u] * by + az[u] * bz;
+                const T xx = pc.h - cs;
+                x2[u] = xx * xx;
+                den[u] = pc.d2 + x2[u];
+            }
+            fm::rcp_v<2>(den, q);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const T term = fcb * (T(1) + pc.c2_over_d2 * x2[u] * q[u]);
+                zt[u] += b != av[u] ? term : T(0);
+            }
+        }
+        // zeta = 0: b = 1, b' = 0 (reading A8); the chain runs on a harmless argument and is dropped
+        bool pos[2];
+        T arg[2], lg[2], tt[2], l1[2], bo[2], den2[2], rq[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) { pos[u] = zt[u] > T(0); arg[u] = pos[u] ? pc.beta * zt[u] : T(1); }
+        fm::log_v<2>(arg, lg, tb);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) arg[u] = pc.n * lg[u];
+        fm::exp_v<2>(arg, tt, tb);                                                   // (beta zeta)^n
+#pragma unroll
+        for (int u = 0; u < 2; ++u) arg[u] = T(1) + tt[u];
+        fm::log_v<2>(arg, l1, tb);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) { den2[u] = (pos[u] ? zt[u] : T(1)) * arg[u]; arg[u] = pc.minus_half_over_n * l1[u]; }
+        fm::exp_v<2>(arg, bo, tb);                                                   // Eq. (3)
+        fm::rcp_v<2>(den2, rq);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (!val[u]) continue;
+            const T bov = pos[u] ? bo[u] : T(1);
+            const T bp = pos[u] ? T(-0.5) * bo[u] * tt[u] * rq[u] : T(0);
+            const T c = s.fc[ca[u]], cp = s.fcp[ca[u]], fR = s.fRD[ca[u]], fA = s.fAh[ca[u]];
+            const TsPair<T> pp = tab.p[ti * NT + (NT > 1 ? (int)((unsigned)s.jj[ca[u]] >> 28) : 0)];
+            const T bfA = bov * fA;
+            U += T(0.5) * c * (fR - bfA);                                                  // U_ia / 2
+            s.fRD[ca[u]] = T(0.5) * (cp * (fR - bfA) + c * (pp.mu * bfA - pp.lambda * fR));   // D
+            s.fAh[ca[u]] = T(-0.5) * c * fA * bp;                                          // h
+        }
     }
 
     // pass 3: P_a = D_a e_a + sum_{b != a} [ (h_a fc_b + h_b fc_a) g' (e_b - cos e_a)/r_a + h_b fc'_a g e_a ]
+    // (two slots a per iteration as in pass 2; b == a is masked)
     T Fx = T(0), Fy = T(0), Fz = T(0);
     T W[9] = {T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
     unsigned long long run = mk;
-    for (int a = 0; a < M; ++a) {
-        const int m = __ffsll((long long)run) - 1;
-        run &= run - 1;
-        const int ca = col + 32 * a;
-        const T ax = s.ex[ca], ay = s.ey[ca], az = s.ez[ca];
-        const T ha = s.fAh[ca], fca = s.fc[ca], cpa = s.fcp[ca], ria = s.rinv[ca];
-        const int ja = s.jj[ca] & 0x0fffffff;
-        const unsigned slot = ps::dense_slot(MASK[ja], (int)REV[(int64_t)m * n + i]);   // dense record layout
-        T ce = s.fRD[ca];                                    // coefficient of e_a
-        T sx = T(0), sy = T(0), sz = T(0);                   // sum of ta * e_b
-        auto fterm = [&](int b) {
+    for (int a0 = 0; a0 < M; a0 += 2) {
+        int av[2], ca[2], ja[2], rv[2];
+        bool val[2];
+        T ax[2], ay[2], az[2], ha[2], fca[2], cpa[2], ria[2], ce[2], sx[2], sy[2], sz[2];
+        unsigned long long mj[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            val[u] = a0 + u < M;
+            av[u] = val[u] ? a0 + u : a0;
+            ca[u] = col + 32 * av[u];
+            const int m = run ? __ffsll((long long)run) - 1 : 0;
+            if (val[u]) run &= run - 1;
+            ja[u] = s.jj[ca[u]] & 0x0fffffff;
+            rv[u] = (int)REV[(int64_t)m * n + i];
+            mj[u] = MASK[ja[u]];
+            ax[u] = s.ex[ca[u]]; ay[u] = s.ey[ca[u]]; az[u] = s.ez[ca[u]];
+            ha[u] = s.fAh[ca[u]]; fca[u] = s.fc[ca[u]]; cpa[u] = s.fcp[ca[u]]; ria[u] = s.rinv[ca[u]];
+            ce[u] = s.fRD[ca[u]];                            // coefficient of e_a
+            sx[u] = T(0); sy[u] = T(0); sz[u] = T(0);        // sum of ta * e_b
+        }
+#pragma unroll 2
+        for (int b = 0; b < M; ++b) {
             const int cb = col + 32 * b;
-            const T bx = s.ex[cb], by = s.ey[cb], bz = s.ez[cb];
-            const T cs = ax * bx + ay * by + az * bz;
-            const T xx = pc.h - cs;
-            const T x2 = xx * xx;
-            const T q = fm::rcp(pc.d2 + x2);
-            const T hb = s.fAh[cb];
-            const T gp = T(-2) * pc.c2 * xx * q * q;         // dg/dcos
-            const T ta = (ha * s.fc[cb] + hb * fca) * gp * ria;
-            ce += hb * cpa * (T(1) + pc.c2_over_d2 * x2 * q) - ta * cs;
-            sx += ta * bx; sy += ta * by; sz += ta * bz;
-        };
-#pragma unroll 2
-        for (int b = 0; b < a; ++b) fterm(b);
-#pragma unroll 2
-        for (int b = a + 1; b < M; ++b) fterm(b);
-        const T px = sx + ce * ax, py = sy + ce * ay, pz = sz + ce * az;
-        rm::store_rec(&Q[slot * (unsigned)n + (unsigned)ja], px, py, pz);
-        Fx += px; Fy += py; Fz += pz;
-        if (virial) {
-            const T r = fm::rcp(ria);
-            const T rx = ax * r, ry = ay * r, rz = az * r;
-            W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
-            W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
-            W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+            const T bx = s.ex[cb], by = s.ey[cb], bz = s.ez[cb], hb = s.fAh[cb], fcb = s.fc[cb];
+            T cs[2], xx[2], x2[2], den[2], q[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                cs[u] = ax[u] * bx + ay[u] * by + az[u] * bz;
+                xx[u] = pc.h - cs[u];
+                x2[u] = xx[u] * xx[u];
+                den[u] = pc.d2 + x2[u];
+            }
+            fm::rcp_v<2>(den, q);
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const bool on = b != av[u];
+                const T gp = T(-2) * pc.c2 * xx[u] * q[u] * q[u];                    // dg/dcos
+                const T ta = on ? (ha[u] * fcb + hb * fca[u]) * gp * ria[u] : T(0);
+                const T cterm = hb * cpa[u] * (T(1) + pc.c2_over_d2 * x2[u] * q[u]) - ta * cs[u];
+                ce[u] += on ? cterm : T(0);
+                sx[u] += ta * bx; sy[u] += ta * by; sz[u] += ta * bz;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (!val[u]) continue;
+            const unsigned slot = ps::dense_slot(mj[u], rv[u]);                      // dense record layout
+            const T px = sx[u] + ce[u] * ax[u], py = sy[u] + ce[u] * ay[u], pz = sz[u] + ce[u] * az[u];
+            rm::store_rec(&Q[slot * (unsigned)n + (unsigned)ja[u]], px, py, pz);
+            Fx += px; Fy += py; Fz += pz;
+            if (virial) {
+                const T r = fm::rcp(ria[u]);
+                const T rx = ax[u] * r, ry = ay[u] * r, rz = az[u] * r;
+                W[0] += rx * px; W[1] += rx * py; W[2] += rx * pz;
+                W[3] += ry * px; W[4] += ry * py; W[5] += ry * pz;
+                W[6] += rz * px; W[7] += rz * py; W[8] += rz * pz;
+            }
         }
     }
     if (pe) pe[i] = (double)U;
