@@ -226,9 +226,9 @@ __device__ __forceinline__ unsigned long long ld_early(const unsigned long long*
 // lane (M_w = largest M in the warp, clamped so that the region fits `pool_slots`; a clamp latches
 // MD_DEV_INRANGE_OVERFLOW and the caller drops the pairs beyond *M_w).  Atoms with t >= na (tile tail) carry
 // mask 0 and sort to the front with M = 0.  Uses four __syncthreads().
-template <int BT>
+template <int BT, class SS>
 __device__ __forceinline__ void
-sort_by_count(SortScratch<BT>& s, unsigned long long my_mask, int pool_slots, int* __restrict__ status,
+sort_by_count(SS& s, unsigned long long my_mask, int pool_slots, int* __restrict__ status,
               int* t_out, unsigned long long* mask_out, int* base_out, int* Mw_out) {
     constexpr int NW = BT / 32;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -291,6 +291,108 @@ sort_by_count(SortScratch<BT>& s, unsigned long long my_mask, int pool_slots, in
         Mw = base < pool_slots ? (pool_slots - base) / 32 : 0;
     }
     *t_out = t; *mask_out = mk; *base_out = base; *Mw_out = Mw;
+}
+
+// The same sort for a tile of 2 * BT atoms and BT threads (scratch: SortScratch<2 * BT>; thread `tid` brings the masks
+// of tile entries tid and BT + tid).  The sorted sequence is cut into 2 * BT / 32 blocks of 32 ranks; warp w takes
+// block w in round 0 and block 2 NW - 1 - w in round 1.  With one block per warp the warp that holds the largest
+// counts decides when the CTA is done (cost grows as M^2 in the Tersoff loop code: the other warps idled a third of
+// the time at the next tile's barrier); a small block plus a large one per warp evens that out, and between the two
+// rounds no CTA barrier is needed: the column region of a warp (sized by the larger of its two blocks) is its own.
+// Returns per round r: tile entry t[r], its mask and the warp's column region (base[r], M_w[r]); *sync_between says
+// whether the CTA must meet at a barrier between the rounds (see below).
+template <int BT, class SS>
+__device__ __forceinline__ void
+sort_by_count_x2(SS& s, const unsigned long long (&my_mask)[2], int pool_slots, int* __restrict__ status,
+                 int (&t_out)[2], unsigned long long (&mask_out)[2], int (&base_out)[2], int (&Mw_out)[2],
+                 bool* sync_between) {
+    constexpr int NW = BT / 32;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    int M[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        M[r] = __popcll(my_mask[r]);
+        if (M[r] > MBINS - 1) { atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW); M[r] = MBINS - 1; }
+        s.mask[r * BT + tid] = my_mask[r];
+    }
+    // per-warp histogram over its 64 entries; `before[r]` = entries of the warp that precede this one inside its bin
+    int mine = 0, mine32 = 0, before[2] = {0, 0};
+    const int blo = __reduce_min_sync(0xffffffffu, min(M[0], M[1])), bhi = __reduce_max_sync(0xffffffffu, max(M[0], M[1]));
+    const unsigned below = (1u << lane) - 1u;
+#pragma unroll 1
+    for (int b = blo; b <= bhi; ++b) {
+        const unsigned v0 = __ballot_sync(0xffffffffu, M[0] == b), v1 = __ballot_sync(0xffffffffu, M[1] == b);
+        const int c = __popc(v0) + __popc(v1);
+        if (b < 32) { if (lane == b) mine = c; } else { if (lane == 0) mine32 = c; }
+        if (M[0] == b) before[0] = __popc(v0 & below);
+        if (M[1] == b) before[1] = __popc(v0) + __popc(v1 & below);
+    }
+    s.cnt[wid][lane] = mine;
+    if (lane == 0) s.cnt[wid][32] = mine32;
+    __syncthreads();
+    if (wid == 0) {                                          // exclusive offsets, bin-major then warp-major
+        int run = 0;
+#pragma unroll 1
+        for (int b0 = 0; b0 < MBINS; b0 += 32) {
+            const int b = b0 + lane;
+            int c[NW], tot = 0;
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { c[w] = b < MBINS ? s.cnt[w][b] : 0; tot += c[w]; }
+            int inc = tot;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += v;
+            }
+            int off = run + inc - tot;
+            if (b < MBINS) {
+#pragma unroll
+                for (int w = 0; w < NW; ++w) { s.cnt[w][b] = off; off += c[w]; }
+            }
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 2; ++r) s.perm[s.cnt[wid][M[r]] + before[r]] = (unsigned short)(r * BT + tid);
+    __syncthreads();
+    // largest count of every block (warp w looks at blocks w and 2 NW - 1 - w)
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int block = r == 0 ? wid : 2 * NW - 1 - wid;
+        const int m = min(__popcll(s.mask[s.perm[block * 32 + lane]]), MBINS - 1);
+        const int wm = __reduce_max_sync(0xffffffffu, m);
+        if (lane == 0) s.wmax[block] = wm;
+    }
+    __syncthreads();
+    // The blocks are in ascending order of M, so the four large ones run side by side in the balanced assignment
+    // and the pool has to hold them together.  If it cannot (hot or strongly disordered inputs), the tile runs as
+    // {two largest, two smallest blocks}, CTA barrier, {the four in the middle}, with the pool divided anew for
+    // each round: about the demand of two tiles of BT atoms.  The choice is the same for every thread of the CTA.
+    int top = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) top += s.wmax[2 * NW - 1 - w];
+    const bool balanced = 32 * top <= pool_slots;
+    *sync_between = !balanced;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        auto block_of = [&](int w) {
+            if (balanced) return r == 0 ? w : 2 * NW - 1 - w;
+            return r == 0 ? (w < NW / 2 ? 2 * NW - 1 - w : NW - 1 - w) : NW / 2 + w;
+        };
+        auto need_of = [&](int w) { return balanced ? s.wmax[2 * NW - 1 - w] : s.wmax[block_of(w)]; };
+        int base = 0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) base += w < wid ? 32 * need_of(w) : 0;
+        int Mw = need_of(wid);
+        if (base + 32 * Mw > pool_slots) {                   // pool exhausted: keep what fits, flag it
+            if (lane == 0) atomicOr(&status[0], MD_DEV_INRANGE_OVERFLOW);
+            Mw = base < pool_slots ? (pool_slots - base) / 32 : 0;
+        }
+        t_out[r] = s.perm[block_of(wid) * 32 + lane];
+        mask_out[r] = s.mask[t_out[r]];
+        base_out[r] = base; Mw_out[r] = Mw;
+    }
 }
 
 }  // namespace ps

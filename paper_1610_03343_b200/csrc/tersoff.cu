@@ -650,7 +650,7 @@ tersoff_binned_cta(int64_t cta, int64_t n, const double* __restrict__ x, const d
 // With one element it only sees the atoms of the long-row bin (k_tersoff_binned takes the others).
 template <class T, int BT, int PCA>
 struct TersoffSortSmem {
-    ps::SortScratch<BT> ss;
+    ps::SortScratch<2 * BT> ss;                              // two rounds per tile with several elements
     T ex[PCA * BT], ey[PCA * BT], ez[PCA * BT], rinv[PCA * BT];
     T fc[PCA * BT], fcp[PCA * BT], fRD[PCA * BT], fAh[PCA * BT];   // fRD: f_R then D; fAh: f_A then h
     int jj[PCA * BT];
@@ -677,18 +677,35 @@ tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, 
     // grid strides over the tiles (a bin may hold few atoms: a grid sized for "all atoms" would mostly launch
     // CTAs that exit at once, 25 us of nothing at 512 000 atoms)
     const int64_t cnt = list ? (int64_t)*count : n;
-    for (int64_t A0 = cta * BT; A0 < cnt; A0 += nctas * BT) {
+    // Several elements: tiles of 2 BT atoms in two rounds per thread (ps::sort_by_count_x2: every warp takes a block
+    // of small and a block of large in-range counts); one element (the tail bin of config 5): BT atoms, one round.
+    constexpr int RT = NT > 1 ? 2 : 1;
+    for (int64_t A0 = cta * (RT * BT); A0 < cnt; A0 += nctas * (RT * BT)) {
     __syncthreads();                                         // the previous tile is done with the scratch
-    const int64_t a0 = A0 + tid < cnt ? (list ? (int64_t)list[A0 + tid] : A0 + tid) : -1;
-    s.ss.atom[tid] = (int)a0;
-    const unsigned long long mask0 = a0 >= 0 ? MASK[a0] : 0ull;   // in-range mask (k_screen wrote it)
-    int t, base, Mw;
-    unsigned long long mk;
-    ps::sort_by_count<BT>(s.ss, mask0, PCA * BT, status, &t, &mk, &base, &Mw);
-    const int M = min(__popcll(mk), Mw);
-    const int64_t i = s.ss.atom[t];
-    if (i < 0) continue;                                     // tile tail (M = 0); the loop's barrier is reached by all
-    const int col = base + lane;                             // slot k of this thread: col + 32 k
+    unsigned long long mask0[RT];
+#pragma unroll
+    for (int r = 0; r < RT; ++r) {
+        const int64_t e = A0 + r * BT + tid;
+        const int64_t a0 = e < cnt ? (list ? (int64_t)list[e] : e) : -1;
+        s.ss.atom[r * BT + tid] = (int)a0;
+        mask0[r] = a0 >= 0 ? MASK[a0] : 0ull;                // in-range mask (k_screen wrote it)
+    }
+    int tv[2], basev[2], Mwv[2];
+    unsigned long long mkv[2];
+    bool sync_between = false;
+    if constexpr (RT == 1) {
+        ps::sort_by_count<BT>(s.ss, mask0[0], PCA * BT, status, &tv[0], &mkv[0], &basev[0], &Mwv[0]);
+    } else {
+        ps::sort_by_count_x2<BT>(s.ss, mask0, PCA * BT, status, tv, mkv, basev, Mwv, &sync_between);
+    }
+#pragma unroll 1
+    for (int rd = 0; rd < RT; ++rd) {
+    if (rd > 0 && sync_between) __syncthreads();             // the pool is divided anew for this round (CTA-uniform)
+    const int col = basev[rd] + lane;                        // slot k of this thread: col + 32 k
+    const unsigned long long mk = mkv[rd];
+    const int M = min(__popcll(mk), Mwv[rd]);
+    const int64_t i = s.ss.atom[tv[rd]];
+    if (i < 0) continue;                                     // tile tail (M = 0); the barriers are reached by all
 
     const int ti = NT > 1 ? types[i] : 0;
     const TsCenter<T> pc = tab.c[ti];
@@ -902,6 +919,7 @@ tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, 
 #pragma unroll
         for (int q = 0; q < 9; ++q) virial[(int64_t)q * n + i] = (double)(T(-0.5) * W[q]);
     }
+    }   // rounds
     }   // tiles
 }
 
