@@ -147,7 +147,8 @@ template <class T>
 __global__ void __launch_bounds__(256, 4)
 k_screen(unsigned n, const double* x, const double* y, const double* z,
          double Lx, double Ly, double Lz, const int32_t* __restrict__ NN, const int32_t* __restrict__ NL,
-         RangeTab<T> rt, const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK, Bins bins) {
+         const __grid_constant__ RangeTab<T> rt,              // indexed in place (a by-value copy lands on the stack)
+         const int32_t* __restrict__ types, unsigned long long* __restrict__ MASK, Bins bins) {
     const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
     int bin = -1;
     // Inside md_nve_run: a programmatic dependent of the fused gather that wrote x, y, z (common.cuh,

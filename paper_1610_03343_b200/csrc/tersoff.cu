@@ -701,10 +701,11 @@ tersoff_sorted_ctas(int64_t cta, int64_t nctas, TersoffSortSmem<T, BT, PCA>& s, 
 #pragma unroll 1
     for (int rd = 0; rd < RT; ++rd) {
     if (rd > 0 && sync_between) __syncthreads();             // the pool is divided anew for this round (CTA-uniform)
-    const int col = basev[rd] + lane;                        // slot k of this thread: col + 32 k
-    const unsigned long long mk = mkv[rd];
-    const int M = min(__popcll(mk), Mwv[rd]);
-    const int64_t i = s.ss.atom[tv[rd]];
+    // (selects, not tv[rd]: a dynamic index would put the four small arrays into local memory)
+    const int col = (rd == 0 ? basev[0] : basev[1]) + lane;  // slot k of this thread: col + 32 k
+    const unsigned long long mk = rd == 0 ? mkv[0] : mkv[1];
+    const int M = min(__popcll(mk), rd == 0 ? Mwv[0] : Mwv[1]);
+    const int64_t i = s.ss.atom[rd == 0 ? tv[0] : tv[1]];
     if (i < 0) continue;                                     // tile tail (M = 0); the barriers are reached by all
 
     const int ti = NT > 1 ? types[i] : 0;
