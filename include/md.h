@@ -158,7 +158,8 @@ int md_nve_run(md_neighbors* nl, int potential, const void* params, int precisio
 
 /* NPT by weak coupling: Berendsen thermostat and barostat, the paper's benchmark ensemble (
  * SURVEY 8(f-3); reading A18).  Each step is a velocity-Verlet step (as md_nve_run) followed by
- *   T = 2 KE / (3 n kB),  P = (2 KE + tr sum_i W_i) / (3 V)      with W_i from the force call (Eq. 29)
+ *   T = 2 KE / (3 n kB),  P = (2 KE + tr sum_i W_i) / (3 V)      with sum_i W_i of Eq. (29), formed as
+ *   -sum_ij r_ij (x) dU_i/dr_ij (the same sum regrouped pair by pair; per-atom W_i is not stored by this call)
  *   v *= sqrt(1 + (dt/tau_T)(T0/T - 1));   x, box *= (1 - beta (dt/tau_P)(P0 - P))^(1/3)
  * T0 in K, tau in fs, P0 in eV/A^3 (1 eV/A^3 = 160.21766 GPa), beta (compressibility) in A^3/eV.
  * box: HOST double[3], read and UPDATED.  T_trace, P_trace: HOST [nsteps] (may be NULL), the values measured

@@ -371,6 +371,12 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
     }
     int rc;
     double* W = nl->npt_w;
+    // The barostat needs the TOTAL virial only.  Summed over the atoms, Eq. (29) regroups into
+    //   sum_i W_i = -1/2 sum_ij r_ij (x) (P_ij - P_ji) = - sum_ij r_ij (x) P_ij = 2 sum_i W_i^own,
+    // W_i^own = -1/2 sum_j r_ij (x) P_ij being what the pair kernel leaves in `virial` (r_ji = -r_ij, i <-> j in the
+    // second term).  So the gather runs forces-only here (160 instead of 512 bytes per atom, no list or neighbour
+    // coordinates) and per-atom W_i is never formed; md_tersoff_force / md_sw_force still deliver it.
+    struct OwnOnly { md_neighbors* h; OwnOnly(md_neighbors* q) : h(q) { h->virial_own_only = 1; } ~OwnOnly() { h->virial_own_only = 0; } } own_only(nl);
     if (!f_valid) {
         if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
@@ -392,7 +398,7 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
         if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, f, hk, sums, s)) != MD_OK) return rc;
         const double ke2 = sums[0] * mass_amu / MD_KAPPA;                 // 2 KE
         const double V = box[0] * box[1] * box[2];
-        const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + sums[1]) / (3.0 * V);
+        const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + 2.0 * sums[1]) / (3.0 * V);   // tr sum W = 2 tr sum W^own
         if (T_trace) T_trace[step - first_step] = T;
         if (P_trace) P_trace[step - first_step] = P;
         lam_p = T > 0 ? sqrt(1.0 + dt_fs / b->tau_T * (b->T0 / T - 1.0)) : 1.0;

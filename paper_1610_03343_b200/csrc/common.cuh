@@ -47,6 +47,8 @@ struct md_neighbors {
     int gather_pdl;         // the last pair launch wants the fused gather as its programmatic dependent (measured per
                             // path: +3 % after k_tersoff_lean, 0 after k_sw_sorted, -6 % after k_tersoff_hot, whose 148
                             // long-running tail CTAs then share their SMs with early-resident gather CTAs)
+    int virial_own_only;    // md_npt_run: the force call leaves only the pair kernel's own half -1/2 sum_j r_ij (x) P_ij in
+                            // `virial` (the gather runs forces-only); the TOTAL virial is twice the sum of the own halves
     int q_dense;            // layout of the records the last pair kernel wrote: 1 = slot counts in-range entries
                             // (sorted kernels, MASK known beforehand), 0 = slot is the list position
     // cell structures

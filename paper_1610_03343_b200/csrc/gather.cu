@@ -210,6 +210,7 @@ k_gather_vv(int64_t n, int K, const Rec* Q, const unsigned long long* MASK, int 
 int md_launch_gather(md_neighbors* nl, int64_t n, const double* x, const double* y, const double* z,
                      const double* vx, const double* vy, const double* vz, const double box[3],
                      int precision, double* f, double* virial, double* heat, const VVFuse* vv, cudaStream_t s) {
+    if (nl->virial_own_only) virial = nullptr;               // see common.cuh: only the total virial is wanted
     if (n == 0 || (!f && !virial && !heat)) return MD_OK;
     ProfScope prof(nl, MD_KIND_GATHER, 1, s);
     if (vv) {
