@@ -31,6 +31,9 @@
  *     neighbours of a 128-atom tile in a shared-memory pool of 128 x 8 (Tersoff) or 128 x 12
  *     (Stillinger-Weber) slots, of which each of the tile's four warps (atoms sorted by in-range count) takes
  *     32 x its largest count: the four largest-per-warp counts must sum to <= 32 (Tersoff) / 48 (SW).
+ *     With several elements (md_tersoff_multi_force) a tile is 256 atoms sorted into eight blocks of 32, taken
+ *     four at a time: the same bound holds for the largest counts of {two largest, two smallest blocks} and of
+ *     the four blocks in the middle.
  *   - There is no CPU fallback: every entry point needs a CUDA device.
  */
 #ifndef MD_H_
