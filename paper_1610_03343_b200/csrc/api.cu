@@ -18,6 +18,7 @@ void free_all(md_neighbors* nl) {
     cudaFree(nl->cell_count); cudaFree(nl->cell_of); cudaFree(nl->rank_in_cell); cudaFree(nl->sorted); cudaFree(nl->sortedf);
     cudaFree(nl->scan_blocks); cudaFree(nl->d_status); cudaFree(nl->e2e); cudaFree(nl->npt_w); cudaFree(nl->npt_part);
     if (nl->h_npt) cudaFreeHost(nl->h_npt);
+    if (nl->npt_event) cudaEventDestroy(nl->npt_event);
     if (nl->h_maxrow) cudaFreeHost(nl->h_maxrow);
     if (nl->ev_list) cudaEventDestroy(nl->ev_list);
     if (nl->ev_fork) cudaEventDestroy(nl->ev_fork);
@@ -367,7 +368,7 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
     }
     if (!nl->npt_part) {
         if (cudaMalloc(&nl->npt_part, sizeof(double) * md_npt_scratch_doubles()) != cudaSuccess ||
-            cudaMallocHost(&nl->h_npt, 6 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+            cudaMallocHost(&nl->h_npt, 8 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
     }
     int rc;
     double* W = nl->npt_w;
@@ -383,27 +384,37 @@ int md_npt_run(md_neighbors* nl, int potential, const void* params, int precisio
                                  nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
     }
     // Per step: kick+drift (with the scaling the step before decided applied first, in the same pass), [rebuild],
-    // force with W, then ONE pass that does the second half-kick and the two sums, two scalars to the host,
-    // lambda and mu for the next kick+drift.  Operation for operation the unfused sequence (kick; sums; scale).
+    // force with the own-half W, then ONE pass that does the second half-kick and the two sums; a one-thread
+    // kernel forms T, P, lambda, mu and the scaled box on the device, and the next step's kick+drift -- which reads
+    // them from there -- is enqueued before the host waits for the copy of that record (its box for the next build and
+    // pair kernel, the two trace values): the round trip to the host overlaps with that pass.
     const double hk = 0.5 * dt_fs * MD_KAPPA / mass_amu;
     double lam_p = 1.0, mu_p = 1.0;
-    for (int step = first_step; step < first_step + nsteps; ++step) {
-        if ((rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s, lam_p, mu_p)) != MD_OK) return rc;
+    bool drift_enqueued = false;
+    const int last = first_step + nsteps - 1;
+    for (int step = first_step; step <= last; ++step) {
+        if (!drift_enqueued &&
+            (rc = md_launch_vv(nl, 0, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, box, s, lam_p, mu_p)) != MD_OK) return rc;
+        drift_enqueued = false;
         if (step % rebuild_every == 0)
             if ((rc = md_build_neighbors(nl, n, x, y, z, box, r_list, stream)) != MD_OK) return rc;
         if (nl->n != n) return MD_ERR_NO_LIST;
         if ((rc = force_dispatch(nl, potential, params, precision, n, x, y, z, nullptr, nullptr, nullptr, box,
                                  nullptr, f, W, nullptr, nullptr, s)) != MD_OK) return rc;
-        double sums[2];
-        if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, f, hk, sums, s)) != MD_OK) return rc;
-        const double ke2 = sums[0] * mass_amu / MD_KAPPA;                 // 2 KE
+        if ((rc = md_launch_npt_sums(nl, n, vx, vy, vz, W, f, hk, mass_amu, dt_fs, box, b, s)) != MD_OK) return rc;
+        if (step < last) {
+            if ((rc = md_launch_vv_dev(nl, n, x, y, z, vx, vy, vz, f, mass_amu, dt_fs, md_npt_scal(nl), s)) != MD_OK) return rc;
+            drift_enqueued = true;
+        }
+        double rec[7];
+        if ((rc = md_npt_sums_wait(nl, rec)) != MD_OK) return rc;
+        const double ke2 = rec[0] * mass_amu / MD_KAPPA;                  // 2 KE
         const double V = box[0] * box[1] * box[2];
-        const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + 2.0 * sums[1]) / (3.0 * V);   // tr sum W = 2 tr sum W^own
+        const double T = ke2 / (3.0 * (double)n * MD_KB), P = (ke2 + 2.0 * rec[1]) / (3.0 * V);   // tr sum W = 2 tr sum W^own
         if (T_trace) T_trace[step - first_step] = T;
         if (P_trace) P_trace[step - first_step] = P;
-        lam_p = T > 0 ? sqrt(1.0 + dt_fs / b->tau_T * (b->T0 / T - 1.0)) : 1.0;
-        mu_p = cbrt(1.0 - b->beta * dt_fs / b->tau_P * (b->P0 - P));
-        for (int a = 0; a < 3; ++a) box[a] *= mu_p;
+        lam_p = rec[2]; mu_p = rec[3];
+        for (int a = 0; a < 3; ++a) box[a] = rec[4 + a];
     }
     if (nsteps > 0 && (rc = md_launch_npt_scale(nl, n, x, y, z, vx, vy, vz, lam_p, mu_p, s)) != MD_OK) return rc;
     return MD_OK;
@@ -434,7 +445,7 @@ int md_nve_heat_run(md_neighbors* nl, int potential, const void* params, int pre
     }
     if (!nl->npt_part) {
         if (cudaMalloc(&nl->npt_part, sizeof(double) * md_npt_scratch_doubles()) != cudaSuccess ||
-            cudaMallocHost(&nl->h_npt, 6 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
+            cudaMallocHost(&nl->h_npt, 8 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MD_ERR_ALLOC; }
     }
     double* J = nl->npt_w;
     double* pe = nl->npt_w + 3 * n;

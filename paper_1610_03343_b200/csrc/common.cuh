@@ -77,7 +77,7 @@ struct md_neighbors {
     size_t ev_used;                                    // events handed out since the last read
     double ms_acc[MD_N_KINDS];
     // Berendsen NPT (md_npt_run): per-atom virial [9][n], reduction scratch, pinned landing zone
-    double* npt_w; int64_t npt_cap; double* npt_part; double* h_npt;
+    double* npt_w; int64_t npt_cap; double* npt_part; double* h_npt; cudaEvent_t npt_event;
     // md_nve_run_host: the velocities travel on a second stream while the list build and the first force
     // evaluation (which need positions only) already run
     cudaStream_t s_copy; cudaEvent_t ev_fork, ev_join;
@@ -180,8 +180,15 @@ int md_launch_vv(md_neighbors* nl, int phase, int64_t n, double* x, double* y, d
                  double lam = 1.0, double mu = 1.0);   // phase 0 only: v *= lam, x *= mu first (Berendsen scaling of md_npt_run)
 const double* md_math_tables();   // device tables of fastmath.cuh for the current device (nullptr on failure)
 int md_launch_probe_fp64(int iters, double* tflops, cudaStream_t s);
+int md_launch_vv_dev(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy, double* vz,
+                     const double* f, double mass, double dt, const double* d_scal, cudaStream_t s);
+// sums, thermostat / barostat factors and the scaled box on the device (d_scal = md_npt_scal(nl)), copy to the host
+// enqueued; md_npt_sums_wait blocks until that copy has arrived: out = {sum v^2, tr sum W^own, lam, mu, Lx, Ly, Lz}
 int md_launch_npt_sums(md_neighbors* nl, int64_t n, double* vx, double* vy, double* vz,
-                       const double* W, const double* f, double hk, double out[2], cudaStream_t s);
+                       const double* W, const double* f, double hk, double mass, double dt, const double box[3],
+                       const md_berendsen_params* b, cudaStream_t s);
+int md_npt_sums_wait(md_neighbors* nl, double out[7]);
+const double* md_npt_scal(md_neighbors* nl);
 int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
                         double* vz, double lam, double mu, cudaStream_t s);
 int md_launch_heat_sums(md_neighbors* nl, int64_t n, const double* vx, const double* vy, const double* vz,

@@ -31,11 +31,22 @@ k_npt_partial(int64_t n, double* __restrict__ vx, double* __restrict__ vy, doubl
         part[2 * blockIdx.x] = ta; part[2 * blockIdx.x + 1] = tb;
     }
 }
-__global__ void k_npt_final(const double* __restrict__ part, double* __restrict__ out) {
+// out = {sum v^2, tr sum W^own, lam, mu, Lx mu, Ly mu, Lz mu} (reading A18; the total virial is twice the
+// sum of the own halves, api.cu md_npt_run).  The factors are formed here so that the next step's kick + drift
+// (k_kick_drift_dev) can start without the host; the host takes lam, mu and the box from this record, not from a
+// computation of its own, so both sides hold the same bits.
+__global__ void k_npt_final(const double* __restrict__ part, double* __restrict__ out, double n_atoms, double mass_over_kappa,
+                            double dt, double bx, double by, double bz, md_berendsen_params b) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double ta = 0.0, tb = 0.0;
     for (int k = 0; k < RED_BLOCKS; ++k) { ta += part[2 * k]; tb += part[2 * k + 1]; }
     out[0] = ta; out[1] = tb;
+    const double ke2 = ta * mass_over_kappa;                                      // 2 KE
+    const double V = bx * by * bz;
+    const double T = ke2 / (3.0 * n_atoms * MD_KB), P = (ke2 + 2.0 * tb) / (3.0 * V);
+    const double lam = T > 0 ? sqrt(1.0 + dt / b.tau_T * (b.T0 / T - 1.0)) : 1.0;
+    const double mu = cbrt(1.0 - b.beta * dt / b.tau_P * (b.P0 - P));
+    out[2] = lam; out[3] = mu; out[4] = bx * mu; out[5] = by * mu; out[6] = bz * mu;
 }
 __global__ void k_npt_scale(int64_t n, double* __restrict__ x, double* __restrict__ y, double* __restrict__ z,
                             double* __restrict__ vx, double* __restrict__ vy, double* __restrict__ vz,
@@ -47,18 +58,25 @@ __global__ void k_npt_scale(int64_t n, double* __restrict__ x, double* __restric
 }
 }  // namespace
 
-// sum v^2 and tr sum W -> HOST out[2]; synchronises the stream
 // f != nullptr: v += hk f first (the velocity-Verlet kick that ends the step), in the same pass
 int md_launch_npt_sums(md_neighbors* nl, int64_t n, double* vx, double* vy, double* vz,
-                       const double* W, const double* f, double hk, double out[2], cudaStream_t s) {
+                       const double* W, const double* f, double hk, double mass, double dt, const double box[3],
+                       const md_berendsen_params* b, cudaStream_t s) {
     ProfScope prof(nl, MD_KIND_INTEGRATE, 2, s);
+    if (!nl->npt_event) MD_CUDA_TRY(cudaEventCreateWithFlags(&nl->npt_event, cudaEventDisableTiming));
+    double* out = nl->npt_part + 2 * RED_BLOCKS;
     k_npt_partial<<<RED_BLOCKS, RED_BT, 0, s>>>(n, vx, vy, vz, W, f, hk, nl->npt_part);
-    k_npt_final<<<1, 32, 0, s>>>(nl->npt_part, nl->npt_part + 2 * RED_BLOCKS);
-    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_npt, nl->npt_part + 2 * RED_BLOCKS, 2 * sizeof(double), cudaMemcpyDeviceToHost, s));
-    MD_CUDA_TRY(cudaStreamSynchronize(s));
-    out[0] = nl->h_npt[0]; out[1] = nl->h_npt[1];
+    k_npt_final<<<1, 32, 0, s>>>(nl->npt_part, out, (double)n, mass / MD_KAPPA, dt, box[0], box[1], box[2], *b);
+    MD_CUDA_TRY(cudaMemcpyAsync(nl->h_npt, out, 7 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    MD_CUDA_TRY(cudaEventRecord(nl->npt_event, s));
     return MD_OK;
 }
+int md_npt_sums_wait(md_neighbors* nl, double out[7]) {
+    MD_CUDA_TRY(cudaEventSynchronize(nl->npt_event));
+    for (int q = 0; q < 7; ++q) out[q] = nl->h_npt[q];
+    return MD_OK;
+}
+const double* md_npt_scal(md_neighbors* nl) { return nl->npt_part + 2 * RED_BLOCKS; }
 int md_launch_npt_scale(md_neighbors* nl, int64_t n, double* x, double* y, double* z, double* vx, double* vy,
                         double* vz, double lam, double mu, cudaStream_t s) {
     ProfScope prof(nl, MD_KIND_INTEGRATE, 1, s);
